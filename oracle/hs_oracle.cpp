@@ -1,0 +1,272 @@
+// =====================================================================================
+// hs_oracle.cpp -- CPU ORACLE for the incoherent 1-D harmonic sum of arXiv 2202.12817.
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code,
+// header, table or helper with the CUDA path (paper_2202_12817_b200/csrc, include/hs.h);
+// the flag values below are restated here on purpose.
+//
+// It is a plain, slow, double-precision restatement of the paper's algorithms, one
+// fundamental (or top) bin at a time, in the paper's order and notation:
+//
+//   * eq. 2   SNR = max_H (X_H - mu_H) / sigma_H; only the max and its H
+//                               are returned per bin.
+//   * Alg. 2 greedy harmonic sum; eq. 5 m = h n + d;
+//                               fundamental-bin selection.
+//   * eq. 3     simple harmonic sum = greedy with the drift held at 0.
+//   * Alg. 1 PRESTO harmonic sum; eq. 4 x[round(h n / H)],
+//                               n = LAST bin of the series; H' in powers of two,
+//                               fundamental + even harmonics.
+//   * PRESTO_all / PRESTO+ (PAPER.md:174, 368): all harmonics / additionally every H' = 1..H.
+//
+// Neither algorithm reaches a plainly-defined result faster -- both are heuristics that
+// choose WHICH bins to add -- so the oracle is the algorithm itself, step by step.
+// Inputs are the caller's fp32 powers; all sums and SNRs are formed in fp64.
+//
+// Readings of the paper adopted here:
+//   R1  every bin n in [0, n_fund) gets an output (eq. 12 counts all bins).
+//   R2  PRESTO computes the SNR once per H', after the inner loop, with mu[H'], sigma[H'].
+//   R3  Round() = round-half-up in exact integers: (2 h n + H') / (2 H').      [parity unpinned]
+//   R4  greedy: order h is evaluated iff m = h n + d <= N-1; a missing second bin (m+1 = N)
+//       never wins; once an order is skipped all later ones are.                [parity unpinned]
+//   R5  H steps in total, harmonic ORDERS 1..H, statistics indexed by order.
+//   R6  CompareSNR keeps the first maximum (strict >); best starts at -inf, no clamp at 0,
+//       so best_h is in [1, H].                                                 [parity unpinned]
+//   R7  fundamental selection on by default; a flag disables it.
+//   R8  mu[h-1], sigma[h-1] are inputs (the statistics of the partial sum at order h).
+//   NEXT-2: an optional per-bin multiplier inv_baseline[] whitens the spectrum; the product
+//       x*inv_baseline is formed in fp32 (one IEEE multiply -- the kernel's precision --
+//       because it decides the greedy comparison), everything after it in fp64.
+//
+// Pins (tests/test_oracle_pins.py, tests/golden/): P1 identity at H = 1, P2 constant
+// spectrum closed form, P3 delta train, P4 the paper's worked index example
+// (PAPER.md:170, 172), P5 brute force on tiny spectra (exact rational rounding; path-tree
+// enumeration), P6 invariants, P7 exact-integer spectra, P8 Exp(1) noise statistics.
+// Parity unpinned by anything the paper prints: R3 (tie rule of Round), R4 (band edge),
+// R6 (tie-breaks); they are fixed by the readings above.
+// =====================================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <thread>
+#include <vector>
+
+namespace {
+
+// Flag values restated from the boundary's documentation (not included from include/hs.h).
+constexpr uint32_t F_NO_FUND_SELECT = 1u << 0;  // greedy: order 1 takes x[n] without looking at x[n+1]
+constexpr uint32_t F_NO_DRIFT = 1u << 1;        // greedy: simple harmonic sum, eq. 3
+constexpr uint32_t F_ALL_HARMONICS = 1u << 2;   // PRESTO_all
+constexpr uint32_t F_ALL_ORDERS = 1u << 3;      // with ALL_HARMONICS: PRESTO+
+
+struct Spectrum {
+    const float* x;        // N powers
+    const float* invb;     // optional per-bin multiplier (may be null)
+    int64_t N;
+    // Power at bin m as the method sees it.
+    double at(int64_t m) const {
+        if (invb) {
+            volatile float p = x[m] * invb[m];   // one fp32 multiply (kernel's precision)
+            return (double)p;
+        }
+        return (double)x[m];
+    }
+};
+
+struct Stats {
+    const float* mu;
+    const float* sigma;
+    double snr(double sum, int order) const {   // eq. 2 term for harmonic order `order` (1-based)
+        return (sum - (double)mu[order - 1]) / (double)sigma[order - 1];
+    }
+};
+
+const double NEG_INF = -std::numeric_limits<double>::infinity();
+
+// ---- Algorithm 2 (greedy) for one fundamental bin n --------------------------------
+// snr_h / bin_h (optional, length H): per-order SNR (NaN if the order was not evaluated)
+// and the bin that was added at that order (-1 if none).
+void greedy_bin(const Spectrum& sp, int H, const Stats& st, uint32_t flags, int64_t n,
+                double* best_out, int32_t* besth_out, uint32_t* path_out,
+                double* snr_h, int64_t* bin_h) {
+    const int64_t N = sp.N;
+    int64_t d = 0;          // drift
+    double sum = 0.0;
+    double best = NEG_INF;  // R6: no clamp at zero
+    int32_t bh = 0;
+    uint32_t path = 0;
+    if (snr_h) for (int h = 0; h < H; ++h) snr_h[h] = std::nan("");
+    if (bin_h) for (int h = 0; h < H; ++h) bin_h[h] = -1;
+    for (int h = 1; h <= H; ++h) {
+        const int64_t m = (int64_t)h * n + d;            // eq. 5
+        if (m > N - 1) break;                            // R4
+        const double xd = sp.at(m);                      // x_d
+        double xd1 = (m + 1 <= N - 1) ? sp.at(m + 1) : NEG_INF;   // x_(d+1); R4
+        if (h == 1 && (flags & F_NO_FUND_SELECT)) xd1 = NEG_INF;  // R7
+        if (flags & F_NO_DRIFT) xd1 = NEG_INF;                    // eq. 3
+        int64_t picked = m;
+        if (xd1 > xd) {                                  // strict >, ties stay
+            d += 1;
+            sum += xd1;
+            path |= (1u << (h - 1));
+            picked = m + 1;
+        } else {
+            sum += xd;
+        }
+        const double s = st.snr(sum, h);                 // CalculateSNR
+        if (snr_h) snr_h[h - 1] = s;
+        if (bin_h) bin_h[h - 1] = picked;
+        if (s > best) { best = s; bh = h; }              // CompareSNR, R6
+    }
+    *best_out = best;
+    *besth_out = bh;
+    if (path_out) *path_out = path;
+}
+
+// ---- Algorithm 1 (PRESTO family) for one top bin n -----------------------------------
+inline bool order_in_set(int Hp, uint32_t flags) {
+    if (flags & F_ALL_ORDERS) return true;               // PRESTO+: every H' = 1..H
+    return (Hp & (Hp - 1)) == 0;                         // H' = 1, 2, 4, ...
+}
+
+inline int64_t presto_index(int h, int Hp, int64_t n) {  // Round(h/H' n), R3
+    return (2 * (int64_t)h * n + Hp) / (2 * (int64_t)Hp);
+}
+
+void presto_bin(const Spectrum& sp, int H, const Stats& st, uint32_t flags, int64_t n,
+                double* best_out, int32_t* besth_out, double* snr_h) {
+    double best = NEG_INF;
+    int32_t bh = 0;
+    if (snr_h) for (int h = 0; h < H; ++h) snr_h[h] = std::nan("");
+    for (int Hp = 1; Hp <= H; ++Hp) {
+        if (!order_in_set(Hp, flags)) continue;
+        // fundamental frequency bin
+        double sum = sp.at(presto_index(1, Hp, n));
+        if (flags & F_ALL_HARMONICS) {
+            for (int h = 2; h <= Hp; ++h) sum += sp.at(presto_index(h, Hp, n));
+        } else {
+            for (int h = 2; h <= Hp; h += 2) sum += sp.at(presto_index(h, Hp, n));
+        }
+        const double s = st.snr(sum, Hp);                // R2: once per H'
+        if (snr_h) snr_h[Hp - 1] = s;
+        if (s > best) { best = s; bh = Hp; }
+    }
+    *best_out = best;
+    *besth_out = bh;
+}
+
+bool bad_common(const float* x, int64_t N, int32_t S, int32_t H, const float* mu, const float* sigma) {
+    if (!x || !mu || !sigma || N < 2 || S < 1 || H < 1 || H > 32) return true;
+    for (int h = 0; h < H; ++h) if (!(sigma[h] > 0.0f)) return true;
+    return false;
+}
+
+template <class F>
+void parallel_for_rows(int32_t S, int64_t n_fund, int n_threads, F&& body) {
+    // split (spectrum, bin-range) work items over threads
+    if (n_threads < 1) n_threads = 1;
+    const int64_t chunk = 1 << 16;
+    const int64_t chunks_per_row = (n_fund + chunk - 1) / chunk;
+    const int64_t total = (int64_t)S * chunks_per_row;
+    auto worker = [&](int t) {
+        for (int64_t w = t; w < total; w += n_threads) {
+            const int32_t s = (int32_t)(w / chunks_per_row);
+            const int64_t lo = (w % chunks_per_row) * chunk;
+            const int64_t hi = (lo + chunk < n_fund) ? lo + chunk : n_fund;
+            body(s, lo, hi);
+        }
+    };
+    if (n_threads == 1) { worker(0); return; }
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t) th.emplace_back(worker, t);
+    for (auto& t : th) t.join();
+}
+
+}  // namespace
+
+extern "C" {
+
+// Greedy harmonic sum (Alg. 2) over a batch.  x: [S][in_stride] fp32 (first N of each row used);
+// inv_baseline: same layout or null; mu/sigma: H floats, index h-1; outputs [S][out_stride]:
+// snr fp64, best_h int32, path uint32 (nullable; bit h-1 set iff the drift grew at order h).
+// Bins n >= n_fund are not written.  Returns 0, or 1 on invalid arguments.
+int hs_oracle_greedy(const float* x, const float* inv_baseline, int64_t N, int32_t S, int64_t in_stride,
+                     int32_t H, const float* mu, const float* sigma, uint32_t flags, int64_t n_fund,
+                     double* snr, int32_t* best_h, uint32_t* path, int64_t out_stride, int32_t n_threads) {
+    if (bad_common(x, N, S, H, mu, sigma) || !snr || !best_h) return 1;
+    if (in_stride < N || out_stride < n_fund || n_fund < 0 || n_fund > N) return 1;
+    const Stats st{mu, sigma};
+    parallel_for_rows(S, n_fund, n_threads, [&](int32_t s, int64_t lo, int64_t hi) {
+        const Spectrum sp{x + (int64_t)s * in_stride, inv_baseline ? inv_baseline + (int64_t)s * in_stride : nullptr, N};
+        for (int64_t n = lo; n < hi; ++n) {
+            const int64_t o = (int64_t)s * out_stride + n;
+            greedy_bin(sp, H, st, flags, n, &snr[o], &best_h[o], path ? &path[o] : nullptr, nullptr, nullptr);
+        }
+    });
+    return 0;
+}
+
+// PRESTO family (Alg. 1) over a batch; same conventions.  Output index n is the TOP bin (R10).
+int hs_oracle_presto(const float* x, const float* inv_baseline, int64_t N, int32_t S, int64_t in_stride,
+                     int32_t H, const float* mu, const float* sigma, uint32_t flags, int64_t n_fund,
+                     double* snr, int32_t* best_h, int64_t out_stride, int32_t n_threads) {
+    if (bad_common(x, N, S, H, mu, sigma) || !snr || !best_h) return 1;
+    if (in_stride < N || out_stride < n_fund || n_fund < 0 || n_fund > N) return 1;
+    if ((flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    const Stats st{mu, sigma};
+    parallel_for_rows(S, n_fund, n_threads, [&](int32_t s, int64_t lo, int64_t hi) {
+        const Spectrum sp{x + (int64_t)s * in_stride, inv_baseline ? inv_baseline + (int64_t)s * in_stride : nullptr, N};
+        for (int64_t n = lo; n < hi; ++n) {
+            const int64_t o = (int64_t)s * out_stride + n;
+            presto_bin(sp, H, st, flags, n, &snr[o], &best_h[o], nullptr);
+        }
+    });
+    return 0;
+}
+
+// One bin at a time, with the per-order detail: used for sampled checks at full size and for the
+// near-tie sets of the acceptance rule.  rows/bins: `count` (spectrum, bin) pairs.
+// snr_h: [count][H] per-order SNR (NaN where the order was not evaluated);
+// bin_h: [count][H] bin added at each order (-1 if none) -- nullable.
+int hs_oracle_greedy_bins(const float* x, const float* inv_baseline, int64_t N, int64_t in_stride, int32_t H,
+                          const float* mu, const float* sigma, uint32_t flags,
+                          const int64_t* rows, const int64_t* bins, int64_t count,
+                          double* snr, int32_t* best_h, uint32_t* path, double* snr_h, int64_t* bin_h) {
+    if (bad_common(x, N, 1, H, mu, sigma) || !rows || !bins || !snr || !best_h) return 1;
+    const Stats st{mu, sigma};
+    for (int64_t i = 0; i < count; ++i) {
+        if (bins[i] < 0 || bins[i] >= N) return 1;
+        const Spectrum sp{x + rows[i] * in_stride, inv_baseline ? inv_baseline + rows[i] * in_stride : nullptr, N};
+        greedy_bin(sp, H, st, flags, bins[i], &snr[i], &best_h[i], path ? &path[i] : nullptr,
+                   snr_h ? snr_h + i * H : nullptr, bin_h ? bin_h + i * H : nullptr);
+    }
+    return 0;
+}
+
+int hs_oracle_presto_bins(const float* x, const float* inv_baseline, int64_t N, int64_t in_stride, int32_t H,
+                          const float* mu, const float* sigma, uint32_t flags,
+                          const int64_t* rows, const int64_t* bins, int64_t count,
+                          double* snr, int32_t* best_h, double* snr_h) {
+    if (bad_common(x, N, 1, H, mu, sigma) || !rows || !bins || !snr || !best_h) return 1;
+    if ((flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    const Stats st{mu, sigma};
+    for (int64_t i = 0; i < count; ++i) {
+        if (bins[i] < 0 || bins[i] >= N) return 1;
+        const Spectrum sp{x + rows[i] * in_stride, inv_baseline ? inv_baseline + rows[i] * in_stride : nullptr, N};
+        presto_bin(sp, H, st, flags, bins[i], &snr[i], &best_h[i], snr_h ? snr_h + i * H : nullptr);
+    }
+    return 0;
+}
+
+// Index helpers exposed so the pins can check them against the paper's worked example
+// (bin 800 is the last element of fundamental 100 at H = 8 and of 200 at H = 4).
+int64_t hs_oracle_presto_index(int32_t h, int32_t Hp, int64_t n) { return presto_index(h, Hp, n); }
+int32_t hs_oracle_presto_order_in_set(int32_t Hp, uint32_t flags) { return order_in_set(Hp, flags) ? 1 : 0; }
+
+int32_t hs_oracle_hardware_threads(void) {
+    unsigned n = std::thread::hardware_concurrency();
+    return n ? (int32_t)n : 1;
+}
+
+}  // extern "C"

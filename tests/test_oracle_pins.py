@@ -1,0 +1,416 @@
+"""Pins for the CPU oracle (oracle/hs_oracle.cpp) -- nothing here touches the CUDA path.
+
+Each test fixes the oracle to something other than itself: values the paper prints
+(tests/golden/), closed forms, brute-force enumeration with independent (exact rational)
+index arithmetic, library routines (numpy gathers/cumsum) for the special cases that reduce
+to them, and invariants the paper states.  Pin numbers follow SURVEY.md section 8(c).
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2202_12817_b200 import inputs
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+NO_FUND_SELECT, NO_DRIFT, ALL_HARMONICS, ALL_ORDERS = 1, 2, 4, 8
+
+
+def _rows(path):
+    out = []
+    with open(path) as f:
+        for line in f:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                out.append([int(t) for t in line.split()])
+    return out
+
+
+def _lin_stats(H, mu1=1.0, sig1=1.0):
+    """mu_h = h mu1, sigma_h = sqrt(h) sig1 (statistics of a sum of h iid terms)."""
+    h = np.arange(1, H + 1, dtype=np.float64)
+    return (h * mu1).astype(np.float32), (np.sqrt(h) * sig1).astype(np.float32)
+
+
+# ------------------------------------------------------------------------------------------
+# P4  the paper's worked index example and order set
+# ------------------------------------------------------------------------------------------
+def test_p4_paper_index_example(oracle_mod):
+    for h, Hp, n, want in _rows(os.path.join(GOLDEN, "presto_index_example.txt")):
+        assert oracle_mod.presto_index(h, Hp, n) == want
+
+
+def test_p4_paper_order_set(oracle_mod):
+    (want,) = _rows(os.path.join(GOLDEN, "presto_orders_H32.txt"))
+    assert oracle_mod.presto_orders(32) == want
+    assert oracle_mod.presto_orders(32, ALL_HARMONICS) == want            # PRESTO_all keeps the order set
+    assert oracle_mod.presto_orders(32, ALL_HARMONICS | ALL_ORDERS) == list(range(1, 33))  # PRESTO+
+    assert oracle_mod.presto_orders(12) == [1, 2, 4, 8]
+
+
+def test_p4_presto_harmonic_set_decoded_from_sums(oracle_mod):
+    """Alg. 1 adds the fundamental and the EVEN harmonics only:
+    HARM(8) = {1,2,4,6,8}.  x[b] = 8^b makes every sum a base-8 numeral whose digits are the
+    multiplicities of the bins that were added; expected bins come from exact Fractions."""
+    N = 17
+    x = np.array([8.0 ** b for b in range(N)], dtype=np.float32)
+    H = 8
+    mu = np.zeros(H, np.float32)
+    sg = np.ones(H, np.float32)
+    for flags, harm in ((0, lambda Hp: [1] + list(range(2, Hp + 1, 2))),
+                        (ALL_HARMONICS, lambda Hp: list(range(1, Hp + 1)))):
+        for n in range(N):
+            r = oracle_mod.presto_bins(x, H, mu, sg, [0], [n], flags)
+            for Hp in (1, 2, 4, 8):
+                digits = [0] * N
+                for h in harm(Hp):
+                    digits[math.floor(Fraction(h * n, Hp) + Fraction(1, 2))] += 1
+                want = sum(c * 8 ** b for b, c in enumerate(digits))
+                assert r["snr_h"][0, Hp - 1] == float(want), (flags, n, Hp)
+            for Hp in (3, 5, 6, 7):
+                assert math.isnan(r["snr_h"][0, Hp - 1])
+
+
+# ------------------------------------------------------------------------------------------
+# P1  H = 1 is the identity up to normalisation
+# ------------------------------------------------------------------------------------------
+def test_p1_identity(oracle_mod):
+    rng = np.random.default_rng(11)
+    x = rng.exponential(1.0, (3, 257)).astype(np.float32)
+    mu = np.array([0.75], np.float32)
+    sg = np.array([1.5], np.float32)
+    ident = (x.astype(np.float64) - 0.75) / 1.5
+    s, b = oracle_mod.presto(x, 1, mu, sg)
+    assert np.array_equal(s, ident) and np.all(b == 1)
+    s, b, p = oracle_mod.greedy(x, 1, mu, sg, NO_FUND_SELECT)
+    assert np.array_equal(s, ident) and np.all(b == 1) and np.all(p == 0)
+    # default greedy: the larger of x[n], x[n+1]; x[N] is absent (R4)
+    s, b, p = oracle_mod.greedy(x, 1, mu, sg)
+    nxt = np.concatenate([x[:, 1:], np.full((3, 1), -np.inf, np.float32)], axis=1)
+    assert np.array_equal(s, (np.maximum(x, nxt).astype(np.float64) - 0.75) / 1.5)
+    assert np.array_equal(p, (nxt > x).astype(np.uint32))
+    assert np.all(b == 1)
+
+
+# ------------------------------------------------------------------------------------------
+# P2  constant spectrum: closed form, sqrt(N_harm) gain
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("c", [3.0, 1.0, 0.25])
+def test_p2_constant_spectrum(oracle_mod, c):
+    N, H = 200, 8
+    x = np.full((1, N), c, np.float32)
+    mu, sg = _lin_stats(H, 1.0, 0.5)
+    s, b, p = oracle_mod.greedy(x, H, mu, sg)
+    assert np.all(p == 0)                                   # ties stay: never shifts
+    n = np.arange(N)
+    k = np.where(n == 0, H, np.minimum(H, (N - 1) // np.maximum(n, 1)))   # evaluated orders
+    if c > 1.0:
+        assert np.array_equal(b[0], k)
+        want = np.sqrt(k.astype(np.float32).astype(np.float64)) * (c - 1.0) / 0.5
+        assert np.allclose(s[0], want, rtol=1e-6)           # sigma_h is an fp32 input
+    elif c == 1.0:
+        assert np.all(s[0] == 0.0) and np.all(b == 1)       # all orders tie at 0: the first wins
+    else:
+        assert np.all(b == 1) and np.allclose(s[0], (c - 1.0) / 0.5)
+    # PRESTO_all: S = H' c exactly; PRESTO (Alg. 1): 1 or 1 + H'/2 terms
+    s, b = oracle_mod.presto(x, H, mu, sg, ALL_HARMONICS)
+    if c > 1.0:
+        assert np.all(b == 8) and np.allclose(s, math.sqrt(8) * (c - 1.0) / 0.5, rtol=1e-6)
+    r = oracle_mod.presto_bins(x, H, np.zeros(H, np.float32), np.ones(H, np.float32), [0] * 3, [5, 77, 199])
+    for Hp, terms in ((1, 1), (2, 2), (4, 3), (8, 5)):
+        assert np.all(r["snr_h"][:, Hp - 1] == terms * c)
+
+
+# ------------------------------------------------------------------------------------------
+# P3  delta train
+# ------------------------------------------------------------------------------------------
+def test_p3_delta_train_greedy(oracle_mod):
+    N, f0, K, A, H = 4096, 37, 8, 10.0, 16
+    x = inputs.delta_train(N, f0, K, A).numpy()[None, :]
+    mu, sg = _lin_stats(H)
+    s, b, p = oracle_mod.greedy(x, H, mu, sg, NO_FUND_SELECT)
+    assert int(np.argmax(s[0])) == f0 and np.count_nonzero(s[0] == s[0].max()) == 1
+    assert b[0, f0] == K and p[0, f0] == 0
+    assert s[0, f0] == pytest.approx((K * A - K) / math.sqrt(K), rel=1e-6)      # (A-1) sqrt(K)
+    # with fundamental selection bin f0-1 follows the train too (drift grows at every order)
+    s, b, p = oracle_mod.greedy(x, H, mu, sg)
+    top = np.flatnonzero(s[0] == s[0].max())
+    assert set(top.tolist()) == {f0 - 1, f0}
+    assert p[0, f0] == 0 and p[0, f0 - 1] == (1 << K) - 1 and b[0, f0 - 1] == K
+
+
+def test_p3_delta_train_presto(oracle_mod):
+    N, f0, K, A, H = 4096, 37, 8, 10.0, 16
+    x = inputs.delta_train(N, f0, K, A).numpy()[None, :]
+    mu, sg = _lin_stats(H)                                  # "h, sqrt(h)" statistics
+    for flags in (ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS):
+        s, b = oracle_mod.presto(x, H, mu, sg, flags)
+        assert int(np.argmax(s[0])) == K * f0               # R10: indexed by the TOP harmonic
+        assert b[0, K * f0] == K
+        assert s[0, K * f0] == pytest.approx((A - 1.0) * math.sqrt(K), rel=1e-6)
+    # Alg. 1 proper (even harmonics, term-count statistics): at n = K f0 the even harmonics of
+    # f0/2 are all K harmonics of f0, so H' = 2K wins with (A K - (1+K)) / sqrt(1+K).
+    mu_t, sg_t = (t.numpy() for t in inputs.exp1_stats("presto", H))
+    s, b = oracle_mod.presto(x, H, mu_t, sg_t)
+    assert b[0, K * f0] == 2 * K
+    assert s[0, K * f0] == pytest.approx((A * K - (1 + K)) / math.sqrt(1 + K), rel=1e-6)
+    assert s[0, K * f0] == pytest.approx(23.6666666, rel=1e-6)
+
+
+# ------------------------------------------------------------------------------------------
+# P5  brute force on tiny spectra
+# ------------------------------------------------------------------------------------------
+def _tiny(seed, N):
+    # many exact ties on purpose (values 0..5) so the tie rules are exercised
+    return np.random.default_rng(seed).integers(0, 6, N).astype(np.float32)
+
+
+@pytest.mark.parametrize("flags", [0, ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS])
+def test_p5_presto_bruteforce_exact_rational(oracle_mod, flags):
+    """eq. 4 with python Fractions for the index and exact integer sums (N <= 64, all H <= 8)."""
+    for seed, N in ((1, 7), (2, 33), (3, 64)):
+        x = _tiny(seed, N)
+        for H in range(1, 9):
+            mu = (0.5 * np.arange(1, H + 1)).astype(np.float32)     # exact in fp32
+            sg = (2.0 ** (np.arange(H) % 3)).astype(np.float32)     # powers of two
+            s, b = oracle_mod.presto(x, H, mu, sg, flags)
+            for n in range(N):
+                best, bh = -math.inf, 0
+                for Hp in range(1, H + 1):
+                    if not (flags & ALL_ORDERS) and (Hp & (Hp - 1)):
+                        continue
+                    hs = range(1, Hp + 1) if flags & ALL_HARMONICS else [1] + list(range(2, Hp + 1, 2))
+                    tot = sum(Fraction(float(x[math.floor(Fraction(h * n, Hp) + Fraction(1, 2))])) for h in hs)
+                    snr = (tot - Fraction(float(mu[Hp - 1]))) / Fraction(float(sg[Hp - 1]))
+                    if snr > best:
+                        best, bh = snr, Hp
+                assert s[0, n] == float(best) and b[0, n] == bh, (seed, H, n)
+
+
+@pytest.mark.parametrize("flags", [0, NO_FUND_SELECT])
+def test_p5_greedy_bruteforce_path_tree(oracle_mod, flags):
+    """Enumerate all 2^H monotone drift paths of the tree (Fig. 4).  Exactly one
+    of them is 'locally greedy' (each step takes the larger child, ties stay); the oracle must
+    return that one, and its partial sums can never beat the best path."""
+    for seed, N, H in ((5, 40, 5), (6, 64, 6), (7, 23, 4)):
+        x = _tiny(seed, N)
+        mu = np.arange(1, H + 1).astype(np.float32)
+        sg = np.ones(H, np.float32)
+        res = oracle_mod.greedy_bins(x, H, mu, sg, [0] * N, list(range(N)), flags)
+        for n in range(N):
+            greedy_paths, best_sum_at = [], [-math.inf] * H
+            for bits in range(1 << H):
+                d, tot, in_tree, locally_greedy, sums = 0, 0.0, True, True, []
+                for h in range(1, H + 1):
+                    m = h * n + d
+                    step = (bits >> (h - 1)) & 1
+                    if m > N - 1:                       # band edge: the path ends here (R4)
+                        in_tree = in_tree and (bits >> (h - 1)) == 0   # canonical: no later steps
+                        break
+                    second = float(x[m + 1]) if m + 1 <= N - 1 else None
+                    if h == 1 and (flags & NO_FUND_SELECT):
+                        second = None                   # the tree has a single child here (R7)
+                    if step and second is None:
+                        in_tree = False
+                        break
+                    want = 1 if (second is not None and second > float(x[m])) else 0
+                    locally_greedy = locally_greedy and (step == want)
+                    tot += second if step else float(x[m])
+                    d += step
+                    sums.append(tot)
+                if not in_tree:
+                    continue
+                for i, t in enumerate(sums):
+                    best_sum_at[i] = max(best_sum_at[i], t)
+                if locally_greedy:
+                    greedy_paths.append((bits, sums))
+            assert len(greedy_paths) == 1, (seed, n)
+            bits, sums = greedy_paths[0]
+            assert res["path"][n] == bits
+            got = res["snr_h"][n] * sg + mu           # partial sums back from the per-order SNRs
+            for i, t in enumerate(sums):
+                assert got[i] == t and t <= best_sum_at[i]
+            assert np.all(np.isnan(res["snr_h"][n][len(sums):]))
+            snrs = [(t - mu[i]) / sg[i] for i, t in enumerate(sums)]
+            assert res["snr"][n] == max(snrs)
+            assert res["best_h"][n] == 1 + snrs.index(max(snrs))      # first maximum (R6)
+
+
+# ------------------------------------------------------------------------------------------
+# Special cases that reduce to library routines
+# ------------------------------------------------------------------------------------------
+def test_simple_hs_equals_numpy_gather_cumsum(oracle_mod):
+    """NO_DRIFT greedy is eq. 3, X[n] = sum_h x[h n]: numpy fancy indexing + cumsum."""
+    rng = np.random.default_rng(21)
+    N, H = 5000, 16
+    x = rng.exponential(1.0, N).astype(np.float32)
+    mu, sg = _lin_stats(H)
+    bins = np.arange(1, (N - 1) // H + 1)                      # all H orders inside the band
+    res = oracle_mod.greedy_bins(x, H, mu, sg, np.zeros_like(bins), bins, NO_DRIFT)
+    idx = bins[:, None] * np.arange(1, H + 1)[None, :]
+    S = np.cumsum(x[idx].astype(np.float64), axis=1)
+    snr_h = (S - mu.astype(np.float64)) / sg.astype(np.float64)
+    assert np.allclose(res["snr_h"], snr_h, rtol=1e-13, atol=1e-13)
+    assert np.array_equal(res["best_h"], 1 + np.argmax(snr_h, axis=1))
+    assert np.all(res["path"] == 0)
+    assert np.array_equal(res["bin_h"], idx)
+
+
+def test_presto_all_on_exact_multiples_equals_simple_hs(oracle_mod):
+    """When H' divides n, h n / H' is an integer, so PRESTO_all at top bin n = H' f adds exactly
+    x[h f], h = 1..H' -- the simple harmonic sum of fundamental f (eq. 3 vs eq. 4)."""
+    rng = np.random.default_rng(22)
+    N, H = 4096, 8
+    x = rng.exponential(1.0, N).astype(np.float32)
+    mu, sg = _lin_stats(H)
+    f = np.arange(1, (N - 1) // H + 1)
+    simple = oracle_mod.greedy_bins(x, H, mu, sg, np.zeros_like(f), f, NO_DRIFT)
+    for Hp in (1, 2, 4, 8):
+        pa = oracle_mod.presto_bins(x, H, mu, sg, np.zeros_like(f), f * Hp, ALL_HARMONICS)
+        assert np.allclose(pa["snr_h"][:, Hp - 1], simple["snr_h"][:, Hp - 1], rtol=1e-13, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------
+# P6  invariants
+# ------------------------------------------------------------------------------------------
+def test_p6_greedy_invariants(oracle_mod):
+    w = inputs.workload("cfg1")
+    x = inputs.generate_row(w, 0).numpy()
+    N, H = x.size, 8
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+    bins = np.arange(0, N, 7)
+    for flags in (0, NO_FUND_SELECT):
+        r = oracle_mod.greedy_bins(x, H, mu, sg, np.zeros_like(bins), bins, flags)
+        for h in range(1, H + 1):
+            d_h = np.array([bin(int(p) & ((1 << h) - 1)).count("1") for p in r["path"]])
+            assert np.all(d_h <= (h if flags == 0 else h - 1))
+            ev = r["bin_h"][:, h - 1] >= 0
+            assert np.array_equal(r["bin_h"][ev, h - 1], (h * bins + d_h)[ev])  # eq. 5
+            assert np.all(r["bin_h"][ev, h - 1] <= N - 1)
+            # R4: evaluated iff h n + d_{h-1} <= N-1
+            d_prev = np.array([bin(int(p) & ((1 << (h - 1)) - 1)).count("1") for p in r["path"]])
+            assert np.array_equal(ev, h * bins + d_prev <= N - 1)
+        assert np.all((r["best_h"] >= 1) & (r["best_h"] <= H))
+        s1 = r["snr_h"][:, 0] * sg[0] + mu[0]
+        assert np.all(s1 >= x[bins] - 1e-6)                                     # S_1 >= x[n]
+
+
+def test_p6_presto_depends_only_on_bins_up_to_n(oracle_mod):
+    rng = np.random.default_rng(31)
+    N, H = 3000, 16
+    x = rng.exponential(1.0, N).astype(np.float32)
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+    s0, b0 = oracle_mod.presto(x, H, mu, sg)
+    cut = 1777
+    y = x.copy()
+    y[cut + 1:] = 1e6
+    s1, b1 = oracle_mod.presto(y, H, mu, sg)
+    assert np.array_equal(s0[0, :cut + 1], s1[0, :cut + 1]) and np.array_equal(b0[0, :cut + 1], b1[0, :cut + 1])
+
+
+def test_p6_power_of_two_scaling_and_batch_independence(oracle_mod):
+    rng = np.random.default_rng(32)
+    S, N, H = 4, 2048, 8
+    x = rng.exponential(1.0, (S, N)).astype(np.float32)
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+    s0, b0, p0 = oracle_mod.greedy(x, H, mu, sg)
+    s1, b1, p1 = oracle_mod.greedy(x * 4, H, mu * 4, sg * 4)
+    assert np.array_equal(s0, s1) and np.array_equal(b0, b1) and np.array_equal(p0, p1)
+    for r in range(S):
+        sr, br, pr = oracle_mod.greedy(x[r], H, mu, sg, n_threads=1)
+        assert np.array_equal(sr[0], s0[r]) and np.array_equal(br[0], b0[r]) and np.array_equal(pr[0], p0[r])
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+    q0, c0 = oracle_mod.presto(x, H, mu, sg)
+    q1, c1 = oracle_mod.presto(x * 0.5, H, mu * 0.5, sg * 0.5)
+    assert np.array_equal(q0, q1) and np.array_equal(c0, c1)
+    # n_fund limits the outputs, values unchanged
+    q2, c2 = oracle_mod.presto(x, H, mu, sg, n_fund=100)
+    assert q2.shape == (S, 100) and np.array_equal(q2, q0[:, :100])
+
+
+def test_r4_band_edge(oracle_mod):
+    """Order h is evaluated iff h n + d <= N-1; the absent bin N never wins."""
+    N, H = 101, 4
+    x = np.zeros(N, np.float32)
+    x[100] = 5.0
+    mu = np.zeros(H, np.float32)
+    sg = np.ones(H, np.float32)
+    r = oracle_mod.greedy_bins(x, H, mu, sg, [0] * 4, [25, 50, 100, 99], NO_FUND_SELECT)
+    # n = 25: orders 1..4 land on 25, 50, 75, 100 (m = 100 = N-1 evaluated, second bin absent)
+    assert np.array_equal(r["bin_h"][0], [25, 50, 75, 100]) and r["snr"][0] == 5.0 and r["best_h"][0] == 4
+    # n = 50: order 2 at m = 100, order 3 would be 150 > N-1: skipped
+    assert np.array_equal(r["bin_h"][1], [50, 100, -1, -1]) and r["best_h"][1] == 2
+    # n = 100: only the fundamental; with selection on, x[N] is absent and cannot win
+    assert np.array_equal(r["bin_h"][2], [100, -1, -1, -1])
+    r2 = oracle_mod.greedy_bins(x, H, mu, sg, [0, 0], [100, 99])
+    assert r2["path"][0] == 0 and r2["snr"][0] == 5.0
+    # n = 99 with selection: picks bin 100 (drift 1); order 2 would start at 199 > N-1
+    assert r2["path"][1] == 1 and np.array_equal(r2["bin_h"][1], [100, -1, -1, -1])
+
+
+# ------------------------------------------------------------------------------------------
+# P8  statistics of the partial sums on Exp(1) noise match the closed forms
+# ------------------------------------------------------------------------------------------
+def test_p8_noise_statistics(oracle_mod):
+    H, N = 16, 1 << 20
+    w = inputs.Workload("noise", 1, N, H, seed=77)
+    x = inputs.generate_row(w, 0).numpy()
+    assert abs(x.mean() - 1.0) < 5.0 / math.sqrt(N) and abs(x.var() - 1.0) < 0.02   # Exp(1)
+    bins = np.arange(64, N // (H + 1), 3)
+    cnt = bins.size
+    zeros = np.zeros_like(bins)
+
+    def check(res, variant, mu, sg, orders):
+        for h in orders:
+            S = res["snr_h"][:, h - 1] * sg[h - 1] + mu[h - 1]
+            var = float(sg[h - 1]) ** 2
+            assert abs(S.mean() - mu[h - 1]) < 6.0 * math.sqrt(var / cnt), (variant, h)
+            assert abs(S.var() / var - 1.0) < 0.06, (variant, h)
+
+    mu, sg = (t.numpy().astype(np.float64) for t in inputs.exp1_stats("greedy", H))
+    check(oracle_mod.greedy_bins(x, H, mu, sg, zeros, bins), "greedy", mu, sg, range(1, H + 1))
+    mu, sg = (t.numpy().astype(np.float64) for t in inputs.exp1_stats("greedy", H, fund_select=False))
+    check(oracle_mod.greedy_bins(x, H, mu, sg, zeros, bins, NO_FUND_SELECT), "greedy_nofs", mu, sg, range(1, H + 1))
+    mu, sg = (t.numpy().astype(np.float64) for t in inputs.exp1_stats("simple", H))
+    check(oracle_mod.greedy_bins(x, H, mu, sg, zeros, bins, NO_DRIFT), "simple", mu, sg, range(1, H + 1))
+    top = bins * H       # PRESTO outputs are indexed by the top bin; keep the bins distinct
+    mu, sg = (t.numpy().astype(np.float64) for t in inputs.exp1_stats("presto", H))
+    check(oracle_mod.presto_bins(x, H, mu, sg, zeros, top), "presto", mu, sg, (1, 2, 4, 8, 16))
+    mu, sg = (t.numpy().astype(np.float64) for t in inputs.exp1_stats("presto_plus", H))
+    check(oracle_mod.presto_bins(x, H, mu, sg, zeros, top, ALL_HARMONICS | ALL_ORDERS), "presto_plus", mu, sg, range(1, H + 1))
+
+
+# ------------------------------------------------------------------------------------------
+# P9 (soft, paper-stated): on a noiseless pulse train greedy recovers what PRESTO+ recovers
+# and the simple sum loses; scalloping keeps sinc(1/2) = 0.637
+# of the amplitude for a half-bin offset ("up to 36% loss").
+# ------------------------------------------------------------------------------------------
+def test_p9_noiseless_pulse_train_soft(oracle_mod):
+    N, H = 1 << 14, 16
+    p = inputs.Pulsar(0, 200.5, 0.04, 8.0, 0.3)
+    re = torch.zeros(N, dtype=torch.float64)
+    im = torch.zeros(N, dtype=torch.float64)
+    inputs._inject(re, im, p)
+    x = (re * re + im * im).to(torch.float32).numpy()
+    assert x[200] / 64.0 == pytest.approx((2.0 / math.pi) ** 2, rel=1e-6)     # |sinc(1/2)|^2 of the power
+    mu, sg = _lin_stats(H, 0.0, 1.0)
+    g, _, _ = oracle_mod.greedy(x, H, mu, sg)
+    s, _, _ = oracle_mod.greedy(x, H, mu, sg, NO_DRIFT)
+    pp, _ = oracle_mod.presto(x, H, mu, sg, ALL_HARMONICS | ALL_ORDERS)
+    assert g.max() >= 0.97 * pp.max()
+    # at the fundamental itself the drift-free sum walks off the peak after a few orders
+    assert s[0, 199:202].max() < 0.9 * g[0, 199:202].max()
+
+
+def test_argument_validation(oracle_mod):
+    x = np.ones(16, np.float32)
+    with pytest.raises(ValueError):
+        oracle_mod.greedy(x, 2, [1, 2], [1, 0])            # sigma must be > 0
+    with pytest.raises(ValueError):
+        oracle_mod.presto(x, 2, [1, 2], [1, 1], ALL_ORDERS)  # ALL_ORDERS needs ALL_HARMONICS
+    with pytest.raises(ValueError):
+        oracle_mod.greedy(x, 33, np.ones(33), np.ones(33))
