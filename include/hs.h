@@ -1,0 +1,152 @@
+/* =====================================================================================
+ * hs.h -- C-ABI boundary of the B200-native incoherent harmonic sum (arXiv 2202.12817).
+ *
+ * The library computes, for a batch of fp32 Fourier power spectra (one per time-series /
+ * DM trial), the per-bin maximum SNR over harmonic counts and the harmonic
+ * count that gave it (eq. 2; "only the highest SNR value is returned for
+ * each element n"), with the partial sums formed either
+ *
+ *   - by the paper's GREEDY algorithm (Alg. 2; eq. 5, PAPER.md:182:
+ *     at order h read x[m], x[m+1] with m = h n + d, add the larger, and if it was the
+ *     second one grow the drift d; fundamental-bin selection), or
+ *   - by the PRESTO-like algorithm (Alg. 1; eq. 4, PAPER.md:138:
+ *     X[n] = sum x[round(h n / H')], n the LAST bin of the series, H' in powers of two,
+ *     fundamental plus even harmonics).
+ *
+ * Every step (gather, select, accumulate, normalise, max/argmax, store) runs in the
+ * library's sm_100a kernels.  There is no CPU fallback.
+ *
+ * Symbols and indexing
+ *   N = n_bins per spectrum, S = n_spectra, x[s][b] the power of spectrum s at bin b,
+ *   H = maximum harmonic order (1..32).  mu[h-1], sigma[h-1] are the mean and standard
+ *   deviation of the partial sum at harmonic order h; the library never
+ *   estimates them ("GetMeanStdev()", is the caller's).
+ *   Outputs are written for every bin n in [0, n_fund) of every spectrum; for the greedy
+ *   form n is the FUNDAMENTAL bin, for the PRESTO form n is the TOP (last-summed) bin
+ *   (PAPER.md:140).
+ *
+ * Exact semantics (readings of the paper):
+ *   greedy, per spectrum and n:   d = 0, sum = 0, best = -inf
+ *     for h = 1..H:  m = h n + d;  stop if m > N-1;
+ *        a = x[m];  b = x[m+1] if m+1 <= N-1 else -inf   (b = -inf at h = 1 under
+ *        HS_GREEDY_NO_FUND_SELECT, and always under HS_GREEDY_NO_DRIFT);
+ *        if b > a { d += 1; sum += b; path |= 1 << (h-1) } else sum += a;
+ *        snr_h = (sum - mu[h-1]) / sigma[h-1];  if snr_h > best { best = snr_h; best_h = h }
+ *   PRESTO, per spectrum and n:   best = -inf
+ *     for H' in 1,2,4,..<=H (every H' = 1..H under HS_PRESTO_ALL_ORDERS):
+ *        sum = sum over h in {1} U {2,4,..,H'} (1..H' under HS_PRESTO_ALL_HARMONICS)
+ *              of x[(2 h n + H') / (2 H')]                  (round half up, exact integers)
+ *        snr = (sum - mu[H'-1]) / sigma[H'-1];  if snr > best { best = snr; best_h = H' }
+ *   With d_inv_baseline != NULL every x[b] above is replaced by the fp32 product
+ *   x[b] * inv_baseline[b] (spectrum whitening supplied by the caller).
+ *   Sums are accumulated in fp32 in the order written above; the SNR is formed as
+ *   (sum - mu) * (1/sigma) in fp32.  Non-finite inputs give unspecified results.
+ *
+ * Memory, ownership, threading
+ *   The caller owns every buffer.  d_* pointers are DEVICE pointers on the plan's device;
+ *   h_* pointers are HOST pointers; mu and sigma are always HOST arrays of H floats, read
+ *   during the call and passed to the kernels by value (no hidden copy, no sync).
+ *   Layout: row-major, spectrum s starts at element s*in_stride (inputs) / s*out_stride
+ *   (outputs).  Device base pointers must be 16-byte aligned and strides multiples of 4
+ *   elements.  Inputs and outputs must not alias.  hs_run_* are asynchronous on the given
+ *   CUDA stream (a cudaStream_t passed as void*; NULL = the legacy default stream) and
+ *   neither allocate nor block.  hs_run_*_host are synchronous: they return when the host
+ *   output arrays are complete.  A plan may be reused for any number of runs but not
+ *   concurrently from two host threads.
+ *
+ * Errors: every entry point returns an hs_status; nothing throws or aborts.  Invalid
+ *   arguments are rejected before any launch (HS_ERR_INVALID_ARG), valid but unimplemented
+ *   combinations give HS_ERR_UNSUPPORTED, CUDA runtime failures HS_ERR_CUDA
+ *   (hs_last_cuda_error() returns the cudaError_t value), allocation failures HS_ERR_ALLOC.
+ * ===================================================================================== */
+#ifndef HS_B200_H_
+#define HS_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hs_plan_s* hs_plan_t;
+
+typedef enum {
+    HS_OK = 0,
+    HS_ERR_INVALID_ARG = 1,
+    HS_ERR_UNSUPPORTED = 2,
+    HS_ERR_ALLOC = 3,
+    HS_ERR_CUDA = 4
+} hs_status;
+
+enum {
+    /* algorithm flags (plan) */
+    HS_GREEDY_NO_FUND_SELECT = 1u << 0, /* order 1 takes x[n] without comparing with x[n+1] (PAPER.md:260 is optional) */
+    HS_GREEDY_NO_DRIFT       = 1u << 1, /* simple harmonic sum, eq. 3: the drift stays 0 */
+    HS_PRESTO_ALL_HARMONICS  = 1u << 2, /* PRESTO_all: sum every harmonic 1..H' */
+    HS_PRESTO_ALL_ORDERS     = 1u << 3, /* with ALL_HARMONICS = PRESTO+: every H' = 1..H */
+    /* tuning knob, not semantics: bits 16..23 select a kernel variant (0 = the library's choice);
+       every variant computes the results defined above */
+    HS_TUNE_SHIFT            = 16,
+    HS_TUNE_MASK             = 0xFFu << 16
+};
+
+/* Create a plan for a batch shape.
+ *   n_bins     N, 2 <= N <= 2^31 - 64
+ *   n_spectra  S >= 1
+ *   H          maximum harmonic order, 1..32
+ *   in_stride  elements between consecutive input spectra (0 = n_bins); >= n_bins, multiple of 4
+ *   out_stride elements between consecutive output rows (0 = n_fund rounded up to 4); >= n_fund, multiple of 4
+ *   n_fund     outputs are computed for n < n_fund (0 = n_bins); <= n_bins
+ *   flags      OR of the enum above; HS_PRESTO_ALL_ORDERS requires HS_PRESTO_ALL_HARMONICS
+ *   device     CUDA device ordinal
+ * The plan owns only small internal state (device properties, launch geometry, and -- once
+ * a *_host entry point has been used -- its staging buffers and streams). */
+hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
+                  int64_t in_stride, int64_t out_stride, int64_t n_fund,
+                  uint32_t flags, int32_t device);
+
+/* Greedy harmonic sum (Alg. 2) on device buffers.
+ *   d_spectra       [S][in_stride] fp32 powers (device)
+ *   d_inv_baseline  NULL, or [S][in_stride] fp32 per-bin multipliers (device)
+ *   mu, sigma       HOST arrays of H floats, entry h-1 for order h; sigma > 0
+ *   d_snr           [S][out_stride] fp32 out: max over h of snr_h
+ *   d_best_h        [S][out_stride] int32 out: the order h (1..H) attaining it (first maximum)
+ *   d_path          NULL, or [S][out_stride] uint32 out: bit h-1 set iff the drift grew at order h
+ *   cuda_stream     cudaStream_t */
+hs_status hs_run_greedy(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
+                        const float* mu, const float* sigma,
+                        float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream);
+
+/* PRESTO-like harmonic sum (Alg. 1 and its _all / + variants per the plan flags) on device
+ * buffers; arguments as above; best_h is the H' attaining the maximum. */
+hs_status hs_run_presto(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
+                        const float* mu, const float* sigma,
+                        float* d_snr, int32_t* d_best_h, void* cuda_stream);
+
+/* The same two operations with HOST buffers (any host memory; page-locked memory copies
+ * fastest).  Spectra are streamed through plan-owned device staging buffers in groups of
+ * rows: host->device copy, kernels, device->host copy, overlapped on internal streams.
+ * Synchronous.  h_inv_baseline and h_path may be NULL. */
+hs_status hs_run_greedy_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline,
+                             const float* mu, const float* sigma,
+                             float* h_snr, int32_t* h_best_h, uint32_t* h_path);
+hs_status hs_run_presto_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline,
+                             const float* mu, const float* sigma,
+                             float* h_snr, int32_t* h_best_h);
+
+/* Number of kernels this plan has launched so far (for bench.py's gpu_launches). */
+int64_t hs_launch_count(hs_plan_t plan);
+
+/* Release the plan and everything it owns.  NULL is accepted. */
+hs_status hs_destroy(hs_plan_t plan);
+
+/* Static description of a status code. */
+const char* hs_status_string(hs_status s);
+
+/* cudaError_t of the most recent HS_ERR_CUDA on this host thread (0 if none). */
+int32_t hs_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HS_B200_H_ */

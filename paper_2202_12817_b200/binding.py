@@ -1,0 +1,157 @@
+"""Thin Python binding of the C-ABI library declared in ``include/hs.h``.
+
+Same names as the C entry points; argument marshalling only (tensor -> pointer, sequence ->
+``float[H]``).  Every step of the method runs inside ``libhs_b200.so``; PyTorch supplies device
+memory and streams.  There is NO fallback: if the library is missing or a call fails, an
+exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libhs_b200.so")
+
+HS_OK, HS_ERR_INVALID_ARG, HS_ERR_UNSUPPORTED, HS_ERR_ALLOC, HS_ERR_CUDA = range(5)
+
+HS_GREEDY_NO_FUND_SELECT = 1 << 0
+HS_GREEDY_NO_DRIFT = 1 << 1
+HS_PRESTO_ALL_HARMONICS = 1 << 2
+HS_PRESTO_ALL_ORDERS = 1 << 3
+HS_TUNE_SHIFT = 16
+
+EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host",
+           "hs_launch_count", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
+
+
+class HsError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = _lib.hs_status_string(status).decode() if _lib is not None else str(status)
+        if status == HS_ERR_CUDA and _lib is not None:
+            msg += f" [cudaError {_lib.hs_last_cuda_error()}]"
+        super().__init__(f"{where}: {msg}")
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load libhs_b200.so (built by ``__graft_entry__.build()`` / ``_build.build()``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2202_12817_b200._build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, u32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint32
+    fp = ctypes.POINTER(ctypes.c_float)
+    lib.hs_plan.argtypes = [ctypes.POINTER(vp), i64, i32, i32, i64, i64, i64, u32, i32]
+    lib.hs_plan.restype = ctypes.c_int
+    lib.hs_run_greedy.argtypes = [vp, vp, vp, fp, fp, vp, vp, vp, vp]
+    lib.hs_run_greedy.restype = ctypes.c_int
+    lib.hs_run_presto.argtypes = [vp, vp, vp, fp, fp, vp, vp, vp]
+    lib.hs_run_presto.restype = ctypes.c_int
+    lib.hs_run_greedy_host.argtypes = [vp, vp, vp, fp, fp, vp, vp, vp]
+    lib.hs_run_greedy_host.restype = ctypes.c_int
+    lib.hs_run_presto_host.argtypes = [vp, vp, vp, fp, fp, vp, vp]
+    lib.hs_run_presto_host.restype = ctypes.c_int
+    lib.hs_launch_count.argtypes = [vp]
+    lib.hs_launch_count.restype = i64
+    lib.hs_destroy.argtypes = [vp]
+    lib.hs_destroy.restype = ctypes.c_int
+    lib.hs_status_string.argtypes = [ctypes.c_int]
+    lib.hs_status_string.restype = ctypes.c_char_p
+    lib.hs_last_cuda_error.argtypes = []
+    lib.hs_last_cuda_error.restype = i32
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != HS_OK:
+        raise HsError(rc, where)
+
+
+def _farr(v: Sequence[float]):
+    vals = [float(t) for t in (v.tolist() if hasattr(v, "tolist") else v)]
+    return (ctypes.c_float * len(vals))(*vals)
+
+
+def _dptr(t: Optional[torch.Tensor], dtype, name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def _hptr(t, dtype, name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if isinstance(t, torch.Tensor):
+        if t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+            raise TypeError(f"{name}: expected a contiguous CPU tensor of {dtype}")
+        return t.data_ptr()
+    raise TypeError(f"{name}: expected a CPU torch tensor")
+
+
+def hs_plan(n_bins: int, n_spectra: int, H: int, in_stride: int = 0, out_stride: int = 0, n_fund: int = 0,
+            flags: int = 0, device: int = 0) -> ctypes.c_void_p:
+    lib = load()
+    plan = ctypes.c_void_p()
+    _check(lib.hs_plan(ctypes.byref(plan), n_bins, n_spectra, H, in_stride, out_stride, n_fund, flags, device), "hs_plan")
+    return plan
+
+
+def hs_run_greedy(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor], mu, sigma,
+                  d_snr: torch.Tensor, d_best_h: torch.Tensor, d_path: Optional[torch.Tensor] = None,
+                  stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_run_greedy(plan, _dptr(d_spectra, torch.float32, "d_spectra"),
+                             _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), _farr(mu), _farr(sigma),
+                             _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                             _dptr(d_path, torch.int32, "d_path"),   # uint32 bit masks held in an int32 tensor
+                             stream), "hs_run_greedy")
+
+
+def hs_run_presto(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor], mu, sigma,
+                  d_snr: torch.Tensor, d_best_h: torch.Tensor, stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_run_presto(plan, _dptr(d_spectra, torch.float32, "d_spectra"),
+                             _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), _farr(mu), _farr(sigma),
+                             _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                             stream), "hs_run_presto")
+
+
+def hs_run_greedy_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best_h, h_path=None) -> None:
+    lib = load()
+    _check(lib.hs_run_greedy_host(plan, _hptr(h_spectra, torch.float32, "h_spectra"),
+                                  _hptr(h_inv_baseline, torch.float32, "h_inv_baseline"), _farr(mu), _farr(sigma),
+                                  _hptr(h_snr, torch.float32, "h_snr"), _hptr(h_best_h, torch.int32, "h_best_h"),
+                                  _hptr(h_path, torch.int32, "h_path")), "hs_run_greedy_host")
+
+
+def hs_run_presto_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best_h) -> None:
+    lib = load()
+    _check(lib.hs_run_presto_host(plan, _hptr(h_spectra, torch.float32, "h_spectra"),
+                                  _hptr(h_inv_baseline, torch.float32, "h_inv_baseline"), _farr(mu), _farr(sigma),
+                                  _hptr(h_snr, torch.float32, "h_snr"), _hptr(h_best_h, torch.int32, "h_best_h")),
+           "hs_run_presto_host")
+
+
+def hs_launch_count(plan) -> int:
+    return int(load().hs_launch_count(plan))
+
+
+def hs_destroy(plan) -> None:
+    _check(load().hs_destroy(plan), "hs_destroy")

@@ -1,0 +1,51 @@
+// Shared device-side definitions of the harmonic-sum kernels (CUDA path only; the CPU oracle
+// under oracle/ shares nothing with this directory).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define HS_MAX_H 32
+
+// Normalisation statistics travel by value as a __grid_constant__ kernel parameter
+// (mu_H, sigma_H of the partial sum of length H; eq. 2 as (sum - mu) * (1/sigma)).
+struct HsStats {
+    float mu[HS_MAX_H];
+    float inv_sigma[HS_MAX_H];
+};
+
+struct HsShape {
+    long long n_bins;      // N
+    long long n_fund;      // outputs for n < n_fund
+    long long in_stride;   // elements between input rows
+    long long out_stride;  // elements between output rows
+    int n_spectra;         // S
+    int H;                 // maximum harmonic order
+    unsigned flags;        // HS_* algorithm flags (hs.h)
+};
+
+struct HsIO {
+    const float* __restrict__ x;         // [S][in_stride]
+    const float* __restrict__ inv_base;  // nullable
+    float* __restrict__ snr;             // [S][out_stride]
+    int* __restrict__ best_h;            // [S][out_stride]
+    unsigned* __restrict__ path;         // nullable (greedy only)
+};
+
+// flag values (mirrors include/hs.h; csrc includes hs.h in hs_api.cu and static_asserts equality)
+#define HSF_NO_FUND_SELECT 1u
+#define HSF_NO_DRIFT 2u
+#define HSF_ALL_HARMONICS 4u
+#define HSF_ALL_ORDERS 8u
+
+#define HS_NEG_INF (__int_as_float(0xff800000))
+
+// eq. 2 term in the library's fp32 form
+__device__ __forceinline__ float hs_snr(float sum, float mu, float inv_sigma) {
+    return __fmul_rn(__fsub_rn(sum, mu), inv_sigma);
+}
+
+// streaming (evict-first) stores for the outputs: they are written once and never re-read, and
+// must not push the L2-resident spectrum out
+__device__ __forceinline__ void st_cs(float* p, float v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs(int* p, int v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs(unsigned* p, unsigned v) { __stcs(p, v); }

@@ -1,0 +1,104 @@
+// Tuned greedy harmonic sum (Alg. 2) for the common configuration:
+// no per-bin baseline, drift tracking on, in-row indices < 2^31.
+//
+// Mapping: a CTA owns a tile of R*BLOCK consecutive fundamentals of
+// one spectrum; thread t runs R independent chains, chain j on fundamental f0 + j*BLOCK + t, so
+// that the 32 lanes of a warp always hold 32 consecutive fundamentals: at order h their pairs
+// x[m], x[m+1] (m = h n + d, eq. 5) sit in the contiguous span [h n0, h (n0+32) + h]
+// and the gather is served at 32-byte sector granularity out of L1/L2.  The grid is
+// spectrum-major (blockIdx.y = spectrum) so a spectrum is swept while it is L2-resident:
+// every bin b is re-read at order h by the fundamentals near b/h.
+// The R chains give the memory system R independent dependent-load chains per thread.
+#pragma once
+#include "hs_common.cuh"
+
+template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH>
+__global__ void __launch_bounds__(BLOCK)
+hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
+    const int s = blockIdx.y;
+    const int N = (int)sh.n_bins;
+    const int last = N - 1;
+    const int n_fund = (int)sh.n_fund;
+    const int f0 = blockIdx.x * (BLOCK * R);
+    const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
+
+    // Orders 1..h_safe need no band-edge test for any fundamental of the tile:
+    // m + 1 = h n + d + 1 <= h (n + 1) + 1 <= last.   Orders above h_top are dead for all of them.
+    const int n_hi = min(f0 + BLOCK * R, n_fund) - 1;           // largest fundamental of the tile
+    const int H = sh.H;
+    int h_safe = (last - 1) / (n_hi + 1);
+    h_safe = min(h_safe, H);
+    const int h_top = (f0 == 0) ? H : min(H, last / f0);
+
+    int n[R], d[R], hn[R], bh[R];
+    float sum[R], best[R];
+    unsigned path[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        n[j] = f0 + j * BLOCK + threadIdx.x;
+        d[j] = 0; hn[j] = 0; bh[j] = 0; sum[j] = 0.f; best[j] = HS_NEG_INF; path[j] = 0;
+    }
+    bool live[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) live[j] = n[j] < n_fund;
+#pragma unroll
+    for (int j = 0; j < R; ++j) if (!live[j]) n[j] = n_hi;       // clamp: harmless duplicate work, no OOB
+
+    int h = 1;
+    // ---- unchecked orders ----
+    for (; h <= h_safe; ++h) {
+        const float mu = st.mu[h - 1], is = st.inv_sigma[h - 1];
+        float a[R], b[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) {
+            hn[j] += n[j];
+            const int m = hn[j] + d[j];
+            a[j] = __ldg(x + m);
+            b[j] = __ldg(x + m + 1);
+        }
+#pragma unroll
+        for (int j = 0; j < R; ++j) {
+            bool shift = b[j] > a[j];
+            if (!FUND_SELECT) shift = shift && (h != 1);
+            d[j] += shift;
+            sum[j] = __fadd_rn(sum[j], shift ? b[j] : a[j]);
+            if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
+            const float snr = hs_snr(sum[j], mu, is);
+            if (snr > best[j]) { best[j] = snr; bh[j] = h; }
+        }
+    }
+    // ---- orders that may cross the band edge for some fundamentals (R4) ----
+    bool alive[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) alive[j] = true;
+    for (; h <= h_top; ++h) {
+        const float mu = st.mu[h - 1], is = st.inv_sigma[h - 1];
+#pragma unroll
+        for (int j = 0; j < R; ++j) {
+            hn[j] += n[j];
+            const int m = hn[j] + d[j];
+            alive[j] = alive[j] && (m <= last);
+            if (alive[j]) {
+                const float a = __ldg(x + m);
+                float b = HS_NEG_INF;
+                if (m + 1 <= last && (FUND_SELECT || h != 1)) b = __ldg(x + m + 1);
+                const bool shift = b > a;
+                d[j] += shift;
+                sum[j] = __fadd_rn(sum[j], shift ? b : a);
+                if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
+                const float snr = hs_snr(sum[j], mu, is);
+                if (snr > best[j]) { best[j] = snr; bh[j] = h; }
+            }
+        }
+    }
+    const long long orow = (long long)s * sh.out_stride;
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        if (live[j]) {
+            const long long o = orow + (f0 + j * BLOCK + threadIdx.x);
+            st_cs(io.snr + o, best[j]);
+            st_cs(io.best_h + o, bh[j]);
+            if (WANT_PATH) st_cs(io.path + o, path[j]);
+        }
+    }
+}

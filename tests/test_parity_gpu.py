@@ -1,0 +1,318 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle on
+the same seeded inputs.  Acceptance rules in tests/parity.py."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2202_12817_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+NO_FUND_SELECT, NO_DRIFT, ALL_HARMONICS, ALL_ORDERS = 1, 2, 4, 8
+GENERIC = 255 << 16          # HS_TUNE value that forces the generic kernels
+
+
+@pytest.fixture(scope="module")
+def hs():
+    from paper_2202_12817_b200 import binding
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    binding.load()                      # fails loudly if libhs_b200.so is missing
+    return binding
+
+
+def run_greedy(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, want_path=True, in_stride=0, out_stride=0):
+    x = torch.as_tensor(x)
+    if x.ndim == 1:
+        x = x[None, :]
+    S, N = x.shape
+    istr = in_stride or ((N + 3) & ~3)
+    nf = n_fund or N
+    ostr = out_stride or ((nf + 3) & ~3)
+    dx = torch.zeros((S, istr), dtype=torch.float32, device="cuda")
+    dx[:, :N] = x.cuda()
+    db = None
+    if inv_baseline is not None:
+        db = torch.ones((S, istr), dtype=torch.float32, device="cuda")
+        db[:, :N] = torch.as_tensor(inv_baseline).reshape(S, N).cuda()
+    snr = torch.full((S, ostr), float("nan"), dtype=torch.float32, device="cuda")
+    bh = torch.full((S, ostr), -7, dtype=torch.int32, device="cuda")
+    path = torch.full((S, ostr), -7, dtype=torch.int32, device="cuda") if want_path else None
+    plan = hs.hs_plan(N, S, H, istr, ostr, n_fund, flags, 0)
+    try:
+        hs.hs_run_greedy(plan, dx, db, mu, sg, snr, bh, path)
+        torch.cuda.synchronize()
+        assert hs.hs_launch_count(plan) >= 1
+    finally:
+        hs.hs_destroy(plan)
+    # nothing outside [0, n_fund) is written
+    assert torch.all(torch.isnan(snr[:, nf:])) and torch.all(bh[:, nf:] == -7)
+    return (snr[:, :nf].cpu().numpy(), bh[:, :nf].cpu().numpy(),
+            path[:, :nf].cpu().numpy() if want_path else None)
+
+
+def run_presto(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, in_stride=0, out_stride=0):
+    x = torch.as_tensor(x)
+    if x.ndim == 1:
+        x = x[None, :]
+    S, N = x.shape
+    istr = in_stride or ((N + 3) & ~3)
+    nf = n_fund or N
+    ostr = out_stride or ((nf + 3) & ~3)
+    dx = torch.zeros((S, istr), dtype=torch.float32, device="cuda")
+    dx[:, :N] = x.cuda()
+    db = None
+    if inv_baseline is not None:
+        db = torch.ones((S, istr), dtype=torch.float32, device="cuda")
+        db[:, :N] = torch.as_tensor(inv_baseline).reshape(S, N).cuda()
+    snr = torch.full((S, ostr), float("nan"), dtype=torch.float32, device="cuda")
+    bh = torch.full((S, ostr), -7, dtype=torch.int32, device="cuda")
+    plan = hs.hs_plan(N, S, H, istr, ostr, n_fund, flags, 0)
+    try:
+        hs.hs_run_presto(plan, dx, db, mu, sg, snr, bh)
+        torch.cuda.synchronize()
+    finally:
+        hs.hs_destroy(plan)
+    assert torch.all(torch.isnan(snr[:, nf:])) and torch.all(bh[:, nf:] == -7)
+    return snr[:, :nf].cpu().numpy(), bh[:, :nf].cpu().numpy()
+
+
+def _int_stats(H):
+    """Integer means and power-of-two sigmas: every SNR is exact in fp32 and fp64 (pin P7)."""
+    mu = np.array([3 * h for h in range(1, H + 1)], np.float32)
+    sg = np.array([2.0 ** ((h % 4) - 1) for h in range(1, H + 1)], np.float32)
+    return mu, sg
+
+
+# ------------------------------------------------------------------------------------------
+# P7: exact-integer spectra -> bit-for-bit agreement (index parity), all kernels, ragged shapes
+# ------------------------------------------------------------------------------------------
+SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (2, 1 << 17)]
+
+
+@pytest.mark.parametrize("tune", [0, 1, 3, 4, 6, 8, 255])
+@pytest.mark.parametrize("H", [1, 8, 13, 32])
+def test_greedy_exact_integer(hs, oracle_mod, tune, H):
+    mu, sg = _int_stats(H)
+    for S, N in SHAPES:
+        x = inputs.integer_spectra(100 + N, S, N, 255).numpy()
+        for flags in (0, NO_FUND_SELECT):
+            s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags)
+            s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16))
+            assert np.array_equal(p.view(np.uint32), p_ref), (S, N, flags)
+            assert np.array_equal(b, b_ref), (S, N, flags)
+            assert np.array_equal(s.astype(np.float64), s_ref), (S, N, flags)
+
+
+@pytest.mark.parametrize("tune", [0, 1, 3, 5, 6, 255])
+@pytest.mark.parametrize("H", [1, 2, 8, 13, 16, 32])
+def test_presto_exact_integer(hs, oracle_mod, tune, H):
+    mu, sg = _int_stats(H)
+    for S, N in SHAPES:
+        x = inputs.integer_spectra(200 + N, S, N, 255).numpy()
+        s_ref, b_ref = oracle_mod.presto(x, H, mu, sg)
+        s, b = run_presto(hs, x, H, mu, sg, tune << 16)
+        assert np.array_equal(b, b_ref), (S, N)
+        assert np.array_equal(s.astype(np.float64), s_ref), (S, N)
+
+
+@pytest.mark.parametrize("flags", [NO_DRIFT, NO_DRIFT | NO_FUND_SELECT])
+def test_simple_hs_exact_integer(hs, oracle_mod, flags):
+    H = 16
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(7, 3, 5003, 255).numpy()
+    s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags)
+    s, b, p = run_greedy(hs, x, H, mu, sg, flags)
+    assert np.all(p == 0) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
+
+
+@pytest.mark.parametrize("flags", [ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS])
+@pytest.mark.parametrize("H", [5, 16, 32])
+def test_presto_variants_exact_integer(hs, oracle_mod, flags, H):
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(8, 2, 6007, 255).numpy()
+    s_ref, b_ref = oracle_mod.presto(x, H, mu, sg, flags)
+    s, b = run_presto(hs, x, H, mu, sg, flags)
+    assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
+
+
+def test_strides_and_n_fund(hs, oracle_mod):
+    H = 8
+    mu, sg = _int_stats(H)
+    S, N = 3, 5000
+    x = inputs.integer_spectra(9, S, N, 255).numpy()
+    for tune in (0, 255):
+        s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, 0, n_fund=1234)
+        s, b, p = run_greedy(hs, x, H, mu, sg, tune << 16, n_fund=1234, in_stride=5008, out_stride=1300)
+        assert np.array_equal(p.view(np.uint32), p_ref) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
+        q_ref, c_ref = oracle_mod.presto(x, H, mu, sg, 0, n_fund=777)
+        q, c = run_presto(hs, x, H, mu, sg, tune << 16, n_fund=777, in_stride=5120, out_stride=780)
+        assert np.array_equal(c, c_ref) and np.array_equal(q.astype(np.float64), q_ref)
+    # without the optional path output
+    s2, b2, _ = run_greedy(hs, x, H, mu, sg, 0, want_path=False)
+    s_ref, b_ref, _ = oracle_mod.greedy(x, H, mu, sg, 0)
+    assert np.array_equal(b2, b_ref) and np.array_equal(s2.astype(np.float64), s_ref)
+
+
+# ------------------------------------------------------------------------------------------
+# The BASELINE.json configurations: tolerance-based acceptance (a)-(c)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tune", [0, 255])
+def test_cfg1_both_variants(hs, oracle_mod, tune):
+    from parity import check_greedy, check_presto
+    w = inputs.workload("cfg1")
+    x = inputs.generate(w).numpy()
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", w.H))
+    s, b, p = run_greedy(hs, x, w.H, mu, sg, tune << 16)
+    r = check_greedy(oracle_mod, x, w.H, mu, sg, 0, s, b, p, T=10.0)
+    # the injected pulsar (r = 1000.5) is detected at its fundamental
+    top = int(np.argmax(s[0]))
+    assert top in (1000, 1001) and s[0, top] > 10.0
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", w.H))
+    s, b = run_presto(hs, x, w.H, mu, sg, tune << 16)
+    check_presto(oracle_mod, x, w.H, mu, sg, 0, s, b, T=10.0)
+    assert r["bh_mismatch"] < 10
+
+
+def test_cfg2_subset(hs, oracle_mod):
+    """configs[1] shape (2^20 bins, H = 16), 6 of its 64 rows incl. rows with injected pulsars."""
+    from parity import check_greedy, check_presto
+    w = inputs.workload("cfg2")
+    rows = sorted({p.spectrum for p in w.pulsars})[:4] + [0, 63]
+    x = torch.stack([inputs.generate_row(w, s, "cuda") for s in rows]).cpu().numpy()
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", w.H))
+    s, b, p = run_greedy(hs, x, w.H, mu, sg)
+    check_greedy(oracle_mod, x, w.H, mu, sg, 0, s, b, p, T=10.0)
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", w.H))
+    s, b = run_presto(hs, x, w.H, mu, sg)
+    check_presto(oracle_mod, x, w.H, mu, sg, 0, s, b, T=10.0)
+
+
+def test_noise_all_flags_tolerance(hs, oracle_mod):
+    from parity import check_greedy, check_presto
+    H = 32
+    w = inputs.Workload("n", 2, 300001, H, seed=41, n_pulsars=3, r_range=(50.0, 5000.0), duty_range=(0.02, 0.1),
+                        amp_range=(6.0, 12.0))
+    x = inputs.generate(w).numpy()
+    for flags, variant, fs in ((0, "greedy", True), (NO_FUND_SELECT, "greedy", False), (NO_DRIFT, "simple", True)):
+        mu, sg = (t.numpy() for t in inputs.exp1_stats(variant, H, fs))
+        s, b, p = run_greedy(hs, x, H, mu, sg, flags)
+        check_greedy(oracle_mod, x, H, mu, sg, flags, s, b, p, T=8.0)
+    for flags, variant in ((0, "presto"), (ALL_HARMONICS, "presto_all"), (ALL_HARMONICS | ALL_ORDERS, "presto_plus")):
+        mu, sg = (t.numpy() for t in inputs.exp1_stats(variant, H))
+        s, b = run_presto(hs, x, H, mu, sg, flags)
+        check_presto(oracle_mod, x, H, mu, sg, flags, s, b, T=8.0)
+
+
+def test_inv_baseline_red_noise(hs, oracle_mod):
+    """configs[3] content at reduced size (NEXT-2): red-noise trend, block-median baseline."""
+    from parity import check_greedy, check_presto
+    H = 32
+    w = inputs.Workload("red", 2, 1 << 17, H, seed=4, n_pulsars=2, r_range=(100.0, 4000.0), duty_range=(0.02, 0.1),
+                        amp_range=(8.0, 12.0), red_noise=True)
+    xt = inputs.generate(w)
+    ib = inputs.block_median_inv_baseline(xt).numpy()
+    x = xt.numpy()
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+    s, b, p = run_greedy(hs, x, H, mu, sg, 0, inv_baseline=ib)
+    check_greedy(oracle_mod, x, H, mu, sg, 0, s, b, p, inv_baseline=ib, T=10.0)
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+    s, b = run_presto(hs, x, H, mu, sg, 0, inv_baseline=ib)
+    check_presto(oracle_mod, x, H, mu, sg, 0, s, b, inv_baseline=ib, T=10.0)
+
+
+# ------------------------------------------------------------------------------------------
+# Host-buffer entry points (the e2e leg of bench.py) and error behaviour
+# ------------------------------------------------------------------------------------------
+def test_host_entry_points(hs, oracle_mod):
+    H = 16
+    mu, sg = _int_stats(H)
+    S, N = 9, 40000
+    x = inputs.integer_spectra(10, S, N, 255)
+    hx = x.pin_memory()
+    snr = torch.empty((S, N), dtype=torch.float32).pin_memory()
+    bh = torch.empty((S, N), dtype=torch.int32).pin_memory()
+    path = torch.empty((S, N), dtype=torch.int32).pin_memory()
+    plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+    try:
+        hs.hs_run_greedy_host(plan, hx, None, mu, sg, snr, bh, path)
+        s_ref, b_ref, p_ref = oracle_mod.greedy(x.numpy(), H, mu, sg)
+        assert np.array_equal(path.numpy().view(np.uint32), p_ref) and np.array_equal(bh.numpy(), b_ref)
+        assert np.array_equal(snr.numpy().astype(np.float64), s_ref)
+        hs.hs_run_presto_host(plan, hx, None, mu, sg, snr, bh)
+        q_ref, c_ref = oracle_mod.presto(x.numpy(), H, mu, sg)
+        assert np.array_equal(bh.numpy(), c_ref) and np.array_equal(snr.numpy().astype(np.float64), q_ref)
+        assert hs.hs_launch_count(plan) >= 2
+    finally:
+        hs.hs_destroy(plan)
+
+
+def test_error_behaviour(hs):
+    N, S, H = 1024, 2, 8
+    x = torch.ones((S, N), device="cuda")
+    snr = torch.empty((S, N), device="cuda")
+    bh = torch.empty((S, N), dtype=torch.int32, device="cuda")
+    mu, sg = _int_stats(H)
+    plan = hs.hs_plan(N, S, H)
+    try:
+        bad_sg = sg.copy(); bad_sg[3] = 0.0
+        with pytest.raises(hs.HsError) as e:
+            hs.hs_run_greedy(plan, x, None, mu, bad_sg, snr, bh)
+        assert e.value.status == hs.HS_ERR_INVALID_ARG
+        with pytest.raises(hs.HsError):
+            hs.hs_run_presto(plan, x.view(-1)[1:-3].view(-1), None, mu, sg, snr, bh)     # misaligned pointer
+        with pytest.raises(hs.HsError):
+            hs.hs_run_greedy(plan, x, None, mu, sg, snr, snr.view(torch.int32))           # aliasing outputs
+        hs.hs_run_greedy(plan, x, None, mu, sg, snr, bh)                                   # the plan is still usable
+        torch.cuda.synchronize()
+        assert torch.all(bh >= 1)
+    finally:
+        hs.hs_destroy(plan)
+    with pytest.raises(hs.HsError):
+        hs.hs_plan(N, S, 64)
+
+
+# ------------------------------------------------------------------------------------------
+# Full size, in the launch configuration bench.py times (configs[2]: 256 x 2^22, H = 32)
+# ------------------------------------------------------------------------------------------
+def test_cfg3_full_size_sampled_rows(hs, oracle_mod):
+    """The whole 4 GiB batch goes through one hs_run_* call each (exactly what bench.py times);
+    rows the oracle can afford are compared element by element, every row is checked for the
+    properties that hold at any size."""
+    from parity import check_greedy, check_presto
+    w = inputs.workload("cfg3")
+    S, N, H = w.n_spectra, w.n_bins, w.H
+    free, _ = torch.cuda.mem_get_info()
+    if free < 20 * (1 << 30):
+        pytest.skip("needs 20 GiB of device memory")
+    x = inputs.generate(w, "cuda")
+    snr = torch.empty((S, N), dtype=torch.float32, device="cuda")
+    bh = torch.empty((S, N), dtype=torch.int32, device="cuda")
+    path = torch.empty((S, N), dtype=torch.int32, device="cuda")
+    pulsar_rows = sorted({p.spectrum for p in w.pulsars})
+    rows = [0, pulsar_rows[0], pulsar_rows[len(pulsar_rows) // 2], S - 1]
+    xs = x[rows].cpu().numpy()
+    plan = hs.hs_plan(N, S, H)
+    try:
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+        hs.hs_run_greedy(plan, x, None, mu, sg, snr, bh, path)
+        torch.cuda.synchronize()
+        assert int(bh.min()) >= 1 and int(bh.max()) <= H and bool(torch.isfinite(snr).all())
+        # S_1 >= x[n]  <=>  best >= (x[n] - mu_1)/sigma_1 (P6), at every bin of every row
+        floor1 = (x - float(mu[0])) / float(sg[0])
+        assert bool((snr >= floor1 - 1e-5 * (floor1.abs() + 1)).all())
+        del floor1
+        # bins n >= N/2 evaluate order 1 only: best_h = 1 and path in {0, 1}
+        assert bool((bh[:, N // 2 + 1:] == 1).all()) and int(path[:, N // 2 + 1:].max()) <= 1
+        check_greedy(oracle_mod, xs, H, mu, sg, 0, snr[rows].cpu().numpy(), bh[rows].cpu().numpy(),
+                     path[rows].cpu().numpy(), T=10.0)
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+        hs.hs_run_presto(plan, x, None, mu, sg, snr, bh)
+        torch.cuda.synchronize()
+        assert int(bh.min()) >= 1 and int(bh.max()) <= H and bool(torch.isfinite(snr).all())
+        # H' = 1 is always a candidate: best >= (x[n] - mu_1)/sigma_1
+        floor1 = (x - float(mu[0])) / float(sg[0])
+        assert bool((snr >= floor1 - 1e-5 * (floor1.abs() + 1)).all())
+        del floor1
+        check_presto(oracle_mod, xs, H, mu, sg, 0, snr[rows].cpu().numpy(), bh[rows].cpu().numpy(), T=10.0)
+    finally:
+        hs.hs_destroy(plan)
