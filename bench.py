@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the harmonic-sum hot path (arXiv 2202.12817) on B200.
+
+One STEP = one pass of the whole hot path over one batch of synthetic
+power spectra: hs_run_greedy (Alg. 2) followed by hs_run_presto (Alg. 1,
+PAPER.md:144-162) on the same batch, i.e. every spectrum bin receives both outputs.
+Workload at N=1: BASELINE.json configs[2] ("cfg3": 256 DM trials x 2^22 fp32 bins, H = 32), the
+configuration the metric is quoted on.  N>1: every rank owns its own 256 spectra (weak scaling,
+no data-path collective: spectra are independent).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `value` = spectrum bins per second with the inputs resident in HBM
+(paper eq. 12, counted once per bin although both forms are computed);
+`e2e` = the same through hs_run_*_host with pinned HOST buffers (H2D + D2H inside the timed region).
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "harmonic-sum spectrum bins/s at H=32 (greedy + PRESTO-like forms per bin)"
+UNIT = "bins/s"
+BYTES_PER_BIN = 12.0          # compulsory HBM bytes per bin and per form: 4 read + 4 + 4 written
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/), keyed by kernel family; None until a capture exists.
+NCU_TRAFFIC_BYTES = {"greedy": None, "presto": None}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg3", help="inputs.workload name (cfg3 = headline)")
+    ap.add_argument("--spectra", type=int, default=0, help="override the number of spectra per rank (0 = workload's)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-spectra", type=int, default=64, help="spectra in the oracle's bounded sample")
+    ap.add_argument("--tune-greedy", type=int, default=0)
+    ap.add_argument("--tune-presto", type=int, default=0)
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy burst)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, reasons, smax, pw = [], set(), None, []
+        try:
+            for line in open(self.path):
+                f = [t.strip() for t in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1])); smax = float(f[2]); pw.append(float(f[3]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            s = sorted(sm)
+            out.update(sm_mhz=s[len(s) // 2], sm_max_mhz=smax, reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw) if pw else None)
+        return out
+
+
+def dist_setup(n_gpus: int):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return rank, local, world
+
+
+def barrier(world):
+    import torch
+    import torch.distributed as dist
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def run_cpu_sample(x_host, H, n_threads=None):
+    """Time the oracle, as it stands, on a [rows, N] float32 numpy sample: greedy then PRESTO."""
+    import oracle
+    from paper_2202_12817_b200 import inputs
+    oracle.build()
+    cores = n_threads or oracle.host_threads()
+    mu_g, sg_g = inputs.exp1_stats("greedy", H)
+    mu_p, sg_p = inputs.exp1_stats("presto", H)
+    t0 = time.perf_counter()
+    oracle.greedy(x_host, H, mu_g.numpy(), sg_g.numpy(), n_threads=cores, want_path=False)
+    t1 = time.perf_counter()
+    oracle.presto(x_host, H, mu_p.numpy(), sg_p.numpy(), n_threads=cores)
+    t2 = time.perf_counter()
+    bins = x_host.shape[0] * x_host.shape[1]
+    return {"bins": bins, "seconds": t2 - t0, "greedy_s": t1 - t0, "presto_s": t2 - t1, "cores": cores}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores, rank 0 only, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import torch
+    from paper_2202_12817_b200 import inputs
+    w = inputs.workload(args.workload)
+    rows = min(args.cpu_spectra, w.n_spectra)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"   # generator only (no method arithmetic)
+    x = inputs.generate(w, device=dev, n_spectra=rows).cpu().numpy()
+    for _ in range(args.warmup):
+        run_cpu_sample(x[:max(1, rows // 8)], w.H)
+    tot, bins, cores = 0.0, 0, 0
+    for _ in range(args.steps):
+        r = run_cpu_sample(x, w.H)
+        tot += r["seconds"]; bins += r["bins"]; cores = r["cores"]
+    value = bins / tot
+    sample = f"first {rows} of {w.n_spectra} spectra of {w.name} ({rows}x{w.n_bins} bins), greedy + PRESTO, fp64"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name}: {w.n_spectra} spectra x {w.n_bins} fp32 bins, H={w.H}, greedy + PRESTO (Alg. 1)",
+                       "step": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_cuda(args):
+    import torch
+    from paper_2202_12817_b200 import binding as hs
+    from paper_2202_12817_b200 import inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    hs.load()
+    rank, local, world = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    w = inputs.workload(args.workload)
+    S = args.spectra or w.n_spectra
+    N, H = w.n_bins, w.H
+    # rank r owns global rows [r*S, (r+1)*S): weak scaling, no exchange
+    x = torch.empty((S, N), dtype=torch.float32, device=dev)
+    for s in range(S):
+        x[s].copy_(inputs.generate_row(w, rank * S + s, dev))
+    snr_g = torch.empty((S, N), dtype=torch.float32, device=dev)
+    bh_g = torch.empty((S, N), dtype=torch.int32, device=dev)
+    snr_p = torch.empty_like(snr_g)
+    bh_p = torch.empty_like(bh_g)
+    mu_g, sg_g = inputs.exp1_stats("greedy", H)
+    mu_p, sg_p = inputs.exp1_stats("presto", H)
+    plan_g = hs.hs_plan(N, S, H, flags=args.tune_greedy << hs.HS_TUNE_SHIFT, device=local)
+    plan_p = hs.hs_plan(N, S, H, flags=args.tune_presto << hs.HS_TUNE_SHIFT, device=local)
+    stream = torch.cuda.current_stream(dev)
+
+    def step(ev=None):
+        if ev is not None:
+            ev[0].record(stream)
+        hs.hs_run_greedy(plan_g, x, None, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
+        if ev is not None:
+            ev[1].record(stream)
+        hs.hs_run_presto(plan_p, x, None, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
+        if ev is not None:
+            ev[2].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    l0 = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p)
+    barrier(world)
+    for k in range(args.steps):
+        step(evs[k])
+    barrier(world)
+    launches = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p) - l0
+    total_ms = evs[0][0].elapsed_time(evs[-1][2])          # device time of exactly K steps
+    g_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    p_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    # clocks: keep the sampler running through a few more device-only steps so short runs still get samples
+    if rank == 0:
+        t_end = time.time() + 1.0
+        while time.time() < t_end:
+            step()
+            torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+
+    from paper_2202_12817_b200.sharding import max_over_ranks
+    total_ms = max_over_ranks(total_ms, dev)
+    g_ms = max_over_ranks(g_ms, dev)
+    p_ms = max_over_ranks(p_ms, dev)
+    bins_step = float(S) * N * world
+    value = bins_step * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the host-buffer entry points (pinned host memory, H2D + D2H timed) ----
+    e2e = None
+    if not args.no_e2e:
+        hx = torch.empty((S, N), dtype=torch.float32, pin_memory=True)
+        hx.copy_(x)
+        hsnr = torch.empty((S, N), dtype=torch.float32, pin_memory=True)
+        hbh = torch.empty((S, N), dtype=torch.int32, pin_memory=True)
+        e_steps = max(1, min(args.steps, 5))
+
+        def e2e_step():
+            hs.hs_run_greedy_host(plan_g, hx, None, mu_g, sg_g, hsnr, hbh, None)
+            hs.hs_run_presto_host(plan_p, hx, None, mu_p, sg_p, hsnr, hbh)
+
+        e2e_step()
+        barrier(world)
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            e2e_step()
+        barrier(world)
+        dt = max_over_ranks(time.perf_counter() - t0, dev)
+        e2e = {"value": bins_step * e_steps / dt, "unit": UNIT, "steps": e_steps,
+               "h2d_bytes_per_step": 2 * S * N * 4, "d2h_bytes_per_step": 2 * S * N * 8,
+               "ms_per_step": 1e3 * dt / e_steps,
+               "note": "hs_run_greedy_host + hs_run_presto_host, pinned host buffers, per rank; PCIe-bound"}
+        del hx, hsnr, hbh
+
+    # ---- roofline of the dominant kernel (HBM-bound: 12 algorithmic bytes per bin and launch) ----
+    peak, peak_src = measured_peak()
+    dom, dom_ms = ("greedy", g_ms) if g_ms >= p_ms else ("presto", p_ms)
+    alg_bytes = BYTES_PER_BIN * S * N
+
+    def roof(ms):
+        a = alg_bytes / (ms * 1e-3) / 1e9
+        return a, a / peak
+
+    a, fr = roof(dom_ms)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": a, "peak": peak, "unit": "GB/s", "frac": fr,
+                "traffic": NCU_TRAFFIC_BYTES[dom], "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": dom_ms,
+                "per_kernel": {"greedy": {"launch_ms": g_ms, "achieved": roof(g_ms)[0], "frac": roof(g_ms)[1],
+                                          "gbins_per_s": S * N / g_ms / 1e6},
+                               "presto": {"launch_ms": p_ms, "achieved": roof(p_ms)[0], "frac": roof(p_ms)[1],
+                                          "gbins_per_s": S * N / p_ms / 1e6}}}
+
+    cpu = None
+    if rank == 0 and not args.no_cpu:
+        rows = min(args.cpu_spectra, S)
+        r = run_cpu_sample(x[:rows].cpu().numpy(), H)
+        cpu = {"value": r["bins"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+               "sample": f"first {rows} of {S} spectra of {w.name} ({rows}x{N} bins), greedy {r['greedy_s']:.2f} s + "
+                         f"PRESTO {r['presto_s']:.2f} s, fp64"}
+    hs.hs_destroy(plan_g)
+    hs.hs_destroy(plan_p)
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"{w.name}: {S} spectra x {N} fp32 bins per GPU, H={H}, greedy (Alg. 2) + PRESTO (Alg. 1) per step",
+                           "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": "inputs (4 GiB) exceed L2; no flush needed",
+                           "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
