@@ -12,6 +12,7 @@
 #include "hs_generic.cuh"
 #include "hs_greedy.cuh"
 #include "hs_presto.cuh"
+#include "hs_presto_smem.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -132,6 +133,33 @@ hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     return HS_OK;
 }
 
+template <int T, int L, int BLOCK, bool BULK>
+hs_status launch_presto_smem_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    constexpr int smem = 4 * hs_presto_span_floats<L>(T);
+    static bool attr_set = false;                       // per instantiation; the attribute is per device function
+    if (!attr_set) {
+        HS_CUDA(cudaFuncSetAttribute(hs_presto_smem_kernel<T, L, BLOCK, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
+    hs_presto_smem_kernel<T, L, BLOCK, BULK><<<grid, BLOCK, smem, stream>>>(sh, st, io);
+    p->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+template <int T, int BLOCK, bool BULK>
+hs_status launch_presto_smem(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    switch (floor_log2(sh.H)) {
+        case 0: return launch_presto_smem_L<T, 0, BLOCK, BULK>(p, sh, st, io, stream);
+        case 1: return launch_presto_smem_L<T, 1, BLOCK, BULK>(p, sh, st, io, stream);
+        case 2: return launch_presto_smem_L<T, 2, BLOCK, BULK>(p, sh, st, io, stream);
+        case 3: return launch_presto_smem_L<T, 3, BLOCK, BULK>(p, sh, st, io, stream);
+        case 4: return launch_presto_smem_L<T, 4, BLOCK, BULK>(p, sh, st, io, stream);
+        default: return launch_presto_smem_L<T, 5, BLOCK, BULK>(p, sh, st, io, stream);
+    }
+}
+
 hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
@@ -145,7 +173,15 @@ hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 4: return launch_presto_tile<128, 1>(p, sh, st, io, stream);
             case 5: return launch_presto_tile<128, 2>(p, sh, st, io, stream);
             case 6: return launch_presto_tile<512, 1>(p, sh, st, io, stream);
-            default: return launch_presto_tile<256, 1>(p, sh, st, io, stream);
+            case 7: return launch_presto_tile<256, 1>(p, sh, st, io, stream);
+            case 10: return launch_presto_smem<1024, 256, true>(p, sh, st, io, stream);
+            case 11: return launch_presto_smem<2048, 256, true>(p, sh, st, io, stream);
+            case 12: return launch_presto_smem<1024, 256, false>(p, sh, st, io, stream);
+            case 13: return launch_presto_smem<2048, 256, false>(p, sh, st, io, stream);
+            case 14: return launch_presto_smem<512, 128, true>(p, sh, st, io, stream);
+            case 15: return launch_presto_smem<1024, 128, true>(p, sh, st, io, stream);
+            case 16: return launch_presto_smem<2048, 512, true>(p, sh, st, io, stream);
+            default: return launch_presto_smem<1024, 256, true>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
