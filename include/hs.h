@@ -87,7 +87,11 @@ enum {
     /* tuning knob, not semantics: bits 16..23 select a kernel variant (0 = the library's choice);
        every variant computes the results defined above */
     HS_TUNE_SHIFT            = 16,
-    HS_TUNE_MASK             = 0xFFu << 16
+    HS_TUNE_MASK             = 0xFFu << 16,
+    /* tuning knob: bits 24..27 = spectra per launch group of the two-pass greedy kernels (0 = the
+       library's choice, sized so that the group stays L2-resident) */
+    HS_CHUNK_SHIFT           = 24,
+    HS_CHUNK_MASK            = 0xFu << 24
 };
 
 /* Create a plan for a batch shape.

@@ -11,6 +11,7 @@
 #include "hs_common.cuh"
 #include "hs_generic.cuh"
 #include "hs_greedy.cuh"
+#include "hs_greedy_mask.cuh"
 #include "hs_presto.cuh"
 #include "hs_presto_smem.cuh"
 
@@ -20,6 +21,9 @@ static_assert(HS_PRESTO_ALL_HARMONICS == HSF_ALL_HARMONICS, "flag mismatch");
 static_assert(HS_PRESTO_ALL_ORDERS == HSF_ALL_ORDERS, "flag mismatch");
 
 namespace {
+
+// the band kernel copies fixed-size mask slots that may run past the end of the last row (never looked at)
+constexpr size_t HS_MASK_SLACK_BYTES = 16384;
 
 thread_local int32_t g_last_cuda_error = 0;
 
@@ -43,6 +47,11 @@ struct hs_plan_s {
     int sm_count;
     int64_t launches;
     HostStage stage;
+    // comparison-mask scratch of the two-pass greedy kernels (hs_greedy_mask.cuh): one bit per bin for
+    // the `chunk` spectra in flight, allocated by hs_plan
+    unsigned* d_mask;
+    int mask_stride;        // 32-bit words per spectrum (multiple of 4)
+    int chunk;              // spectra per (mask, gather) launch pair: their spectra stay L2-resident
 };
 
 namespace {
@@ -62,11 +71,11 @@ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 
 hs_status fill_stats(const hs_plan_s* p, const float* mu, const float* sigma, HsStats* st) {
     if (!mu || !sigma) return HS_ERR_INVALID_ARG;
-    for (int h = 0; h < HS_MAX_H; ++h) { st->mu[h] = 0.f; st->inv_sigma[h] = 1.f; }
+    for (int h = 0; h < HS_MAX_H; ++h) { st->nmis[h] = 0.f; st->inv_sigma[h] = 1.f; }
     for (int h = 0; h < p->shape.H; ++h) {
         if (!(sigma[h] > 0.f) || !(sigma[h] < INFINITY) || !(mu[h] == mu[h])) return HS_ERR_INVALID_ARG;
-        st->mu[h] = mu[h];
         st->inv_sigma[h] = 1.0f / sigma[h];     // correctly rounded fp32 reciprocal
+        st->nmis[h] = -(mu[h] * st->inv_sigma[h]);
     }
     return HS_OK;
 }
@@ -91,10 +100,71 @@ hs_status launch_greedy_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     return HS_OK;
 }
 
+// band-specialised mask form (hs_greedy_mask.cuh): per chunk of spectra, one launch writes the comparison
+// mask and the top band's outputs, one launch does the other fundamentals
+template <int BLOCK, int R, int HD, bool FS, bool WP>
+void launch_greedy_band_chunk(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, int n_top, cudaStream_t stream) {
+    dim3 mgrid((unsigned)((p->mask_stride + 31) / 32), (unsigned)sh.n_spectra);
+    hs_cmp_mask_kernel<256, FS, WP><<<mgrid, 256, 0, stream>>>(sh, st, io, p->d_mask, p->mask_stride, n_top);
+    p->launches += 1;
+    const int n_end = (int)std::min<long long>(sh.n_fund, n_top);
+    if (n_end > 0) {
+        const int tile = BLOCK * R;
+        dim3 grid((unsigned)((n_end + tile - 1) / tile), (unsigned)sh.n_spectra);
+        const int smem = 4 * hs_gb_off<BLOCK * R>(sh.H + 1);      // mask spans of every order a tile can reach
+        static bool attr_set = false;                             // per instantiation
+        if (!attr_set) {
+            cudaFuncSetAttribute(hs_greedy_band_kernel<BLOCK, R, HD, FS, WP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 4 * hs_gb_off<BLOCK * R>(HS_MAX_H + 1));
+            attr_set = true;
+        }
+        hs_greedy_band_kernel<BLOCK, R, HD, FS, WP><<<grid, BLOCK, smem, stream>>>(sh, st, io, p->d_mask, p->mask_stride, n_end);
+        p->launches += 1;
+    }
+}
+
+template <int BLOCK, int R, int HD>
+hs_status launch_greedy_band(hs_plan_s* p, const HsShape& full, const HsStats& st, const HsIO& io0, cudaStream_t stream) {
+    const bool fs = !(full.flags & HS_GREEDY_NO_FUND_SELECT);
+    const bool wp = io0.path != nullptr;
+    // fundamentals n >= n_top have exactly one order: 2 n > N - 1
+    const int n_top = (full.H == 1) ? 0 : (int)((full.n_bins - 1) / 2 + 1);
+    for (int s0 = 0; s0 < full.n_spectra; s0 += p->chunk) {
+        HsShape sh = full;
+        sh.n_spectra = std::min(p->chunk, full.n_spectra - s0);
+        HsIO io = io0;
+        io.x += (long long)s0 * full.in_stride;
+        io.snr += (long long)s0 * full.out_stride;
+        io.best_h += (long long)s0 * full.out_stride;
+        if (wp) io.path += (long long)s0 * full.out_stride;
+        if (fs && wp) launch_greedy_band_chunk<BLOCK, R, HD, true, true>(p, sh, st, io, n_top, stream);
+        else if (fs && !wp) launch_greedy_band_chunk<BLOCK, R, HD, true, false>(p, sh, st, io, n_top, stream);
+        else if (!fs && wp) launch_greedy_band_chunk<BLOCK, R, HD, false, true>(p, sh, st, io, n_top, stream);
+        else launch_greedy_band_chunk<BLOCK, R, HD, false, false>(p, sh, st, io, n_top, stream);
+    }
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
 hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
     const bool fast_ok = !io.inv_base && !(sh.flags & HS_GREEDY_NO_DRIFT) && sh.n_bins <= (1ll << 31) - 64 && p->tune != 255;
+    if (fast_ok && p->d_mask && sh.n_bins <= (1ll << 30)) {
+        switch (p->tune) {
+            case 20: return launch_greedy_band<256, 1, 2>(p, sh, st, io, stream);
+            case 21: return launch_greedy_band<256, 2, 2>(p, sh, st, io, stream);
+            case 22: return launch_greedy_band<256, 4, 2>(p, sh, st, io, stream);
+            case 23: return launch_greedy_band<128, 2, 2>(p, sh, st, io, stream);
+            case 24: return launch_greedy_band<128, 4, 2>(p, sh, st, io, stream);
+            case 25: return launch_greedy_band<256, 2, 0>(p, sh, st, io, stream);
+            case 26: return launch_greedy_band<256, 2, 4>(p, sh, st, io, stream);
+            case 27: return launch_greedy_band<128, 4, 4>(p, sh, st, io, stream);
+            case 28: return launch_greedy_band<256, 4, 4>(p, sh, st, io, stream);
+            case 29: return launch_greedy_band<512, 2, 2>(p, sh, st, io, stream);
+            default: break;
+        }
+    }
     if (fast_ok) {
         switch (p->tune) {
             case 1: return launch_greedy_tile<256, 1>(p, sh, st, io, stream);
@@ -301,7 +371,7 @@ hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
     if (in_stride == 0) in_stride = (n_bins + 3) & ~3ll;
     if (out_stride == 0) out_stride = (n_fund + 3) & ~3ll;
     if (in_stride < n_bins || out_stride < n_fund || (in_stride & 3) || (out_stride & 3)) return HS_ERR_INVALID_ARG;
-    const uint32_t known = HS_GREEDY_NO_FUND_SELECT | HS_GREEDY_NO_DRIFT | HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS | HS_TUNE_MASK;
+    const uint32_t known = HS_GREEDY_NO_FUND_SELECT | HS_GREEDY_NO_DRIFT | HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS | HS_TUNE_MASK | HS_CHUNK_MASK;
     if (flags & ~known) return HS_ERR_INVALID_ARG;
     if ((flags & HS_PRESTO_ALL_ORDERS) && !(flags & HS_PRESTO_ALL_HARMONICS)) return HS_ERR_INVALID_ARG;
     if (device < 0) return HS_ERR_INVALID_ARG;
@@ -318,11 +388,29 @@ hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
     p->shape.out_stride = out_stride;
     p->shape.n_spectra = n_spectra;
     p->shape.H = H;
-    p->shape.flags = flags & ~HS_TUNE_MASK;
+    p->shape.flags = flags & ~(HS_TUNE_MASK | HS_CHUNK_MASK);
     p->tune = (flags & HS_TUNE_MASK) >> HS_TUNE_SHIFT;
     p->device = device;
     p->sm_count = sms;
     p->launches = 0;
+    p->d_mask = nullptr;
+    p->mask_stride = 0;
+    p->chunk = 0;
+    if (n_bins <= (1ll << 30) && !(flags & HS_GREEDY_NO_DRIFT)) {
+        // spectra per launch pair: keep the chunk's spectra (and the outputs streaming past them) inside L2
+        int l2 = 0;
+        cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, device);
+        const long long row_bytes = in_stride * 4;
+        long long chunk = (flags & HS_CHUNK_MASK) >> HS_CHUNK_SHIFT;
+        if (chunk == 0) chunk = std::max(1ll, std::min(8ll, ((long long)l2 / 2) / std::max(1ll, row_bytes)));
+        chunk = std::min<long long>(chunk, n_spectra);
+        p->chunk = (int)chunk;
+        p->mask_stride = (int)((((n_bins + 31) / 32) + 3) & ~3ll);
+        cudaError_t e = cudaSetDevice(device);
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_mask, (size_t)p->chunk * p->mask_stride * 4 + HS_MASK_SLACK_BYTES);
+        if (e == cudaSuccess) e = cudaMemset(p->d_mask, 0, (size_t)p->chunk * p->mask_stride * 4 + HS_MASK_SLACK_BYTES);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); delete p; return HS_ERR_ALLOC; }
+    }
     *plan = p;
     return HS_OK;
 }
@@ -363,9 +451,10 @@ int64_t hs_launch_count(hs_plan_t plan) { return plan ? plan->launches : -1; }
 
 hs_status hs_destroy(hs_plan_t plan) {
     if (!plan) return HS_OK;
-    if (plan->stage.ready) {
+    if (plan->stage.ready || plan->d_mask) {
         cudaSetDevice(plan->device);
-        free_stage(plan->stage);
+        if (plan->stage.ready) free_stage(plan->stage);
+        if (plan->d_mask) cudaFree(plan->d_mask);
     }
     delete plan;
     return HS_OK;

@@ -7,10 +7,12 @@
 #define HS_MAX_H 32
 
 // Normalisation statistics travel by value as a __grid_constant__ kernel parameter
-// (mu_H, sigma_H of the partial sum of length H; eq. 2 as (sum - mu) * (1/sigma)).
+// (mu_H, sigma_H of the partial sum of length H).  Eq. 2, (sum - mu)/sigma, is formed
+// as ONE fused multiply-add, sum * (1/sigma) + (-mu/sigma), with both constants rounded once on
+// the host: index h-1 holds order h.
 struct HsStats {
-    float mu[HS_MAX_H];
-    float inv_sigma[HS_MAX_H];
+    float nmis[HS_MAX_H];        // -mu * (1/sigma)
+    float inv_sigma[HS_MAX_H];   // 1/sigma
 };
 
 struct HsShape {
@@ -40,8 +42,8 @@ struct HsIO {
 #define HS_NEG_INF (__int_as_float(0xff800000))
 
 // eq. 2 term in the library's fp32 form
-__device__ __forceinline__ float hs_snr(float sum, float mu, float inv_sigma) {
-    return __fmul_rn(__fsub_rn(sum, mu), inv_sigma);
+__device__ __forceinline__ float hs_snr(float sum, float nmis, float inv_sigma) {
+    return __fmaf_rn(sum, inv_sigma, nmis);
 }
 
 // streaming (evict-first) stores for the outputs: they are written once and never re-read, and

@@ -39,7 +39,7 @@ hs_greedy_generic_kernel(const __grid_constant__ HsShape sh, const __grid_consta
         d += shift;
         sum = __fadd_rn(sum, shift ? b : a);
         path |= (unsigned)shift << (h - 1);
-        const float snr = hs_snr(sum, st.mu[h - 1], st.inv_sigma[h - 1]);
+        const float snr = hs_snr(sum, st.nmis[h - 1], st.inv_sigma[h - 1]);
         if (snr > best) { best = snr; bh = h; }                   // first maximum wins (R6)
     }
     const long long o = (long long)s * sh.out_stride + n;
@@ -68,7 +68,7 @@ hs_presto_generic_kernel(const __grid_constant__ HsShape sh, const __grid_consta
         const int step = all_h ? 1 : 2;
         for (int h = 2; h <= Hp; h += step)
             sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, (2ll * h * n + Hp) / den));
-        const float snr = hs_snr(sum, st.mu[Hp - 1], st.inv_sigma[Hp - 1]);  // once per H' (R2)
+        const float snr = hs_snr(sum, st.nmis[Hp - 1], st.inv_sigma[Hp - 1]);  // once per H' (R2)
         if (snr > best) { best = snr; bh = Hp; }
     }
     const long long o = (long long)s * sh.out_stride + n;

@@ -47,7 +47,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     int h = 1;
     // ---- unchecked orders ----
     for (; h <= h_safe; ++h) {
-        const float mu = st.mu[h - 1], is = st.inv_sigma[h - 1];
+        const float nmis = st.nmis[h - 1], is = st.inv_sigma[h - 1];
         float a[R], b[R];
 #pragma unroll
         for (int j = 0; j < R; ++j) {
@@ -63,7 +63,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             d[j] += shift;
             sum[j] = __fadd_rn(sum[j], shift ? b[j] : a[j]);
             if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
-            const float snr = hs_snr(sum[j], mu, is);
+            const float snr = hs_snr(sum[j], nmis, is);
             if (snr > best[j]) { best[j] = snr; bh[j] = h; }
         }
     }
@@ -72,7 +72,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 #pragma unroll
     for (int j = 0; j < R; ++j) alive[j] = true;
     for (; h <= h_top; ++h) {
-        const float mu = st.mu[h - 1], is = st.inv_sigma[h - 1];
+        const float nmis = st.nmis[h - 1], is = st.inv_sigma[h - 1];
 #pragma unroll
         for (int j = 0; j < R; ++j) {
             hn[j] += n[j];
@@ -86,7 +86,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
                 d[j] += shift;
                 sum[j] = __fadd_rn(sum[j], shift ? b : a);
                 if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
-                const float snr = hs_snr(sum[j], mu, is);
+                const float snr = hs_snr(sum[j], nmis, is);
                 if (snr > best[j]) { best[j] = snr; bh[j] = h; }
             }
         }

@@ -18,7 +18,7 @@ __device__ __forceinline__ void hs_presto_one(const float* __restrict__ x, const
                                               float& best, int& bh) {
     // level 0: H' = 1
     float S = __ldg(x + n);
-    best = hs_snr(S, st.mu[0], st.inv_sigma[0]);
+    best = hs_snr(S, st.nmis[0], st.inv_sigma[0]);
     bh = 1;
 #pragma unroll
     for (int L = 1; L <= LOG2H; ++L) {
@@ -30,7 +30,7 @@ __device__ __forceinline__ void hs_presto_one(const float* __restrict__ x, const
 #pragma unroll
         for (int h = 6; h < Hp; h += 4) add = __fadd_rn(add, __ldg(x + ((h * n + half) >> L)));
         S = __fadd_rn(S, add);
-        const float snr = hs_snr(S, st.mu[Hp - 1], st.inv_sigma[Hp - 1]);
+        const float snr = hs_snr(S, st.nmis[Hp - 1], st.inv_sigma[Hp - 1]);
         if (snr > best) { best = snr; bh = Hp; }
     }
 }

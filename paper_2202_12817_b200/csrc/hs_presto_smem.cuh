@@ -177,7 +177,7 @@ hs_presto_smem_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         const int qs = NW * i;                         // q = w + qs; the k*qs part is an immediate
         int r = 0;
         float S = sm[a[r++] + 32 * qs];               // H' = 1: x[n]
-        float best = hs_snr(S, st.mu[0], st.inv_sigma[0]);
+        float best = hs_snr(S, st.nmis[0], st.inv_sigma[0]);
         int bh = 1;
 #pragma unroll
         for (int l = 1; l <= L; ++l) {
@@ -187,7 +187,7 @@ hs_presto_smem_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 #pragma unroll
             for (int h = 6; h < Hp; h += 4) add = __fadd_rn(add, sm[a[r++] + h * sc * Q * qs]);   // h = 2 mod 4
             S = __fadd_rn(S, add);
-            const float snr = hs_snr(S, st.mu[Hp - 1], st.inv_sigma[Hp - 1]);
+            const float snr = hs_snr(S, st.nmis[Hp - 1], st.inv_sigma[Hp - 1]);
             if (snr > best) { best = snr; bh = Hp; }
         }
         const int n = n0 + 32 * (w + qs) + lane;

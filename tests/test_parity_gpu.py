@@ -89,7 +89,12 @@ def _int_stats(H):
 SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (2, 1 << 17)]
 
 
-@pytest.mark.parametrize("tune", [0, 1, 3, 4, 6, 8, 255])
+# tune word: kernel variant in bits 16..23 (20..27 = two-pass comparison-mask kernels), spectra per launch
+# group in bits 24..27
+GREEDY_TUNES = [0, 1, 3, 4, 6, 8, 255, 20, 22 | (2 << 8), 24 | (1 << 8), 25, 26, 27 | (3 << 8), 29]
+
+
+@pytest.mark.parametrize("tune", GREEDY_TUNES)
 @pytest.mark.parametrize("H", [1, 8, 13, 32])
 def test_greedy_exact_integer(hs, oracle_mod, tune, H):
     mu, sg = _int_stats(H)
