@@ -14,6 +14,7 @@
 #include "hs_greedy_mask.cuh"
 #include "hs_presto.cuh"
 #include "hs_presto_smem.cuh"
+#include "hs_presto_rows.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -230,6 +231,34 @@ hs_status launch_presto_smem(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     }
 }
 
+template <int L, int W, bool BULK>
+hs_status launch_presto_rows_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    constexpr int smem = 4 * hs_rows::smem_words(L, W);
+    static bool attr_set = false;                       // per instantiation
+    if (!attr_set) {
+        HS_CUDA(cudaFuncSetAttribute(hs_presto_rows_kernel<L, W, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    constexpr int T = hs_rows::WT * W;
+    dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
+    hs_presto_rows_kernel<L, W, BULK><<<grid, 32 * W, smem, stream>>>(sh, st, io);
+    p->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+template <int W, bool BULK>
+hs_status launch_presto_rows(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    switch (floor_log2(sh.H)) {
+        case 0: return launch_presto_rows_L<0, W, BULK>(p, sh, st, io, stream);
+        case 1: return launch_presto_rows_L<1, W, BULK>(p, sh, st, io, stream);
+        case 2: return launch_presto_rows_L<2, W, BULK>(p, sh, st, io, stream);
+        case 3: return launch_presto_rows_L<3, W, BULK>(p, sh, st, io, stream);
+        case 4: return launch_presto_rows_L<4, W, BULK>(p, sh, st, io, stream);
+        default: return launch_presto_rows_L<5, W, BULK>(p, sh, st, io, stream);
+    }
+}
+
 hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
@@ -251,6 +280,11 @@ hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 14: return launch_presto_smem<512, 128, true>(p, sh, st, io, stream);
             case 15: return launch_presto_smem<1024, 128, true>(p, sh, st, io, stream);
             case 16: return launch_presto_smem<2048, 512, true>(p, sh, st, io, stream);
+            case 30: return launch_presto_rows<4, true>(p, sh, st, io, stream);
+            case 31: return launch_presto_rows<2, true>(p, sh, st, io, stream);
+            case 32: return launch_presto_rows<3, true>(p, sh, st, io, stream);
+            case 33: return launch_presto_rows<4, false>(p, sh, st, io, stream);
+            case 34: return launch_presto_rows<1, true>(p, sh, st, io, stream);
             default: return launch_presto_smem<1024, 256, true>(p, sh, st, io, stream);
         }
     }
