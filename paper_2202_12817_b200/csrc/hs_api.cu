@@ -15,6 +15,7 @@
 #include "hs_presto.cuh"
 #include "hs_presto_smem.cuh"
 #include "hs_presto_rows.cuh"
+#include "hs_presto_pipe.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -231,31 +232,64 @@ hs_status launch_presto_smem(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     }
 }
 
-template <int L, int W, bool BULK>
+template <int L, int W, bool BULK, int NE>
 hs_status launch_presto_rows_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     constexpr int smem = 4 * hs_rows::smem_words(L, W);
     static bool attr_set = false;                       // per instantiation
     if (!attr_set) {
-        HS_CUDA(cudaFuncSetAttribute(hs_presto_rows_kernel<L, W, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        HS_CUDA(cudaFuncSetAttribute(hs_presto_rows_kernel<L, W, BULK, NE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     constexpr int T = hs_rows::WT * W;
     dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
-    hs_presto_rows_kernel<L, W, BULK><<<grid, 32 * W, smem, stream>>>(sh, st, io);
+    hs_presto_rows_kernel<L, W, BULK, NE><<<grid, (NE < 0 ? 64 : 32) * W, smem, stream>>>(sh, st, io);
     p->launches += 1;
     HS_CUDA(cudaGetLastError());
     return HS_OK;
 }
 
-template <int W, bool BULK>
+template <int W, bool BULK, int NE>
 hs_status launch_presto_rows(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     switch (floor_log2(sh.H)) {
-        case 0: return launch_presto_rows_L<0, W, BULK>(p, sh, st, io, stream);
-        case 1: return launch_presto_rows_L<1, W, BULK>(p, sh, st, io, stream);
-        case 2: return launch_presto_rows_L<2, W, BULK>(p, sh, st, io, stream);
-        case 3: return launch_presto_rows_L<3, W, BULK>(p, sh, st, io, stream);
-        case 4: return launch_presto_rows_L<4, W, BULK>(p, sh, st, io, stream);
-        default: return launch_presto_rows_L<5, W, BULK>(p, sh, st, io, stream);
+        case 0: return launch_presto_rows_L<0, W, BULK, NE>(p, sh, st, io, stream);
+        case 1: return launch_presto_rows_L<1, W, BULK, NE>(p, sh, st, io, stream);
+        case 2: return launch_presto_rows_L<2, W, BULK, NE>(p, sh, st, io, stream);
+        case 3: return launch_presto_rows_L<3, W, BULK, NE>(p, sh, st, io, stream);
+        case 4: return launch_presto_rows_L<4, W, BULK, NE>(p, sh, st, io, stream);
+        default: return launch_presto_rows_L<5, W, BULK, NE>(p, sh, st, io, stream);
+    }
+}
+
+template <int L, int NWARP>
+hs_status launch_presto_pipe_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    constexpr int smem = 4 * NWARP * hs_rows::smem_words(L, 1);
+    static int ctas_per_sm = 0;                         // per instantiation
+    if (!ctas_per_sm) {
+        HS_CUDA(cudaFuncSetAttribute(hs_presto_pipe_kernel<L, NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int nb = 0;
+        HS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, hs_presto_pipe_kernel<L, NWARP>, 32 * NWARP, smem));
+        ctas_per_sm = std::max(1, nb);
+    }
+    const long long tiles_per_row = (sh.n_fund + 511) / 512;
+    const long long total = tiles_per_row * sh.n_spectra;
+    if (total > 0x7fffffffll) return HS_ERR_UNSUPPORTED;
+    const long long want = (total + NWARP - 1) / NWARP;
+    const unsigned grid = (unsigned)std::min<long long>(want, (long long)p->sm_count * ctas_per_sm);
+    hs_presto_pipe_kernel<L, NWARP><<<grid, 32 * NWARP, smem, stream>>>(sh, st, io, (int)tiles_per_row, (int)total);
+    p->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+template <int NWARP>
+hs_status launch_presto_pipe(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    switch (floor_log2(sh.H)) {
+        case 0: return launch_presto_pipe_L<0, NWARP>(p, sh, st, io, stream);
+        case 1: return launch_presto_pipe_L<1, NWARP>(p, sh, st, io, stream);
+        case 2: return launch_presto_pipe_L<2, NWARP>(p, sh, st, io, stream);
+        case 3: return launch_presto_pipe_L<3, NWARP>(p, sh, st, io, stream);
+        case 4: return launch_presto_pipe_L<4, NWARP>(p, sh, st, io, stream);
+        default: return launch_presto_pipe_L<5, NWARP>(p, sh, st, io, stream);
     }
 }
 
@@ -280,12 +314,14 @@ hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 14: return launch_presto_smem<512, 128, true>(p, sh, st, io, stream);
             case 15: return launch_presto_smem<1024, 128, true>(p, sh, st, io, stream);
             case 16: return launch_presto_smem<2048, 512, true>(p, sh, st, io, stream);
-            case 30: return launch_presto_rows<4, true>(p, sh, st, io, stream);
-            case 31: return launch_presto_rows<2, true>(p, sh, st, io, stream);
-            case 32: return launch_presto_rows<3, true>(p, sh, st, io, stream);
-            case 33: return launch_presto_rows<4, false>(p, sh, st, io, stream);
-            case 34: return launch_presto_rows<1, true>(p, sh, st, io, stream);
-            default: return launch_presto_smem<1024, 256, true>(p, sh, st, io, stream);
+            case 30: return launch_presto_rows<4, true, 8>(p, sh, st, io, stream);
+            case 31: return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
+            case 33: return launch_presto_rows<2, false, 8>(p, sh, st, io, stream);
+            case 40: return launch_presto_pipe<4>(p, sh, st, io, stream);
+            case 50: return launch_presto_rows<2, true, -8>(p, sh, st, io, stream);
+            case 35: return launch_presto_rows<2, true, 16>(p, sh, st, io, stream);
+
+            default: return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);

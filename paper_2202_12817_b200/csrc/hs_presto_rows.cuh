@@ -56,17 +56,17 @@ __host__ __device__ constexpr int row_off(int kk, int e) { return (kk * e + 16) 
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-// add the term of fraction KK to the accumulators of outputs e = 8 GRP + u, u = 0..7
+// add the term of fraction KK to the accumulators of outputs e = E0 + u, u = 0..NE-1
 // (FIRST: they are set, not added to)
-template <int KK, int GRP, bool FIRST>
-__device__ __forceinline__ void add_terms(const float* __restrict__ row, float (&acc)[8]) {
+template <int KK, int E0, int NE, bool FIRST>
+__device__ __forceinline__ void add_terms(const float* __restrict__ row, float (&acc)[NE]) {
     if (KK == 1) {                                       // one element for the whole lane
         const float v = row[0];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) acc[u] = FIRST ? v : __fadd_rn(acc[u], v);
+        for (int u = 0; u < NE; ++u) acc[u] = FIRST ? v : __fadd_rn(acc[u], v);
         return;
     }
-    constexpr int lo = row_off(KK, 8 * GRP), hi = row_off(KK, 8 * GRP + 7);
+    constexpr int lo = row_off(KK, E0), hi = row_off(KK, E0 + NE - 1);
     constexpr int A = (KK % 8 == 0) ? 4 : (KK % 4 == 0) ? 2 : 1;     // words the row start is aligned to
     constexpr int lo_al = lo & ~(A - 1);
     constexpr int nvec = (hi - lo_al) / A + 1;
@@ -84,8 +84,8 @@ __device__ __forceinline__ void add_terms(const float* __restrict__ row, float (
         }
     }
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
-        const float v = t[row_off(KK, 8 * GRP + u) - lo_al];
+    for (int u = 0; u < NE; ++u) {
+        const float v = t[row_off(KK, E0 + u) - lo_al];
         acc[u] = FIRST ? v : __fadd_rn(acc[u], v);
     }
 }
@@ -152,67 +152,71 @@ __device__ __forceinline__ const float* row_ptr(const float* __restrict__ sm, in
 }
 
 // S += add, SNR at H' = HP (once per H', reading R2), strict > keeps the first maximum (R6)
-template <int HP>
-__device__ __forceinline__ void close_level(const HsStats& st, float (&S)[8], const float (&add)[8], float (&best)[8], int (&bh)[8]) {
+template <int HP, int NE>
+__device__ __forceinline__ void close_level(const HsStats& st, float (&S)[NE], const float (&add)[NE], float (&best)[NE], int (&bh)[NE]) {
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
+    for (int u = 0; u < NE; ++u) {
         S[u] = __fadd_rn(S[u], add[u]);
         const float snr = hs_snr(S[u], st.nmis[HP - 1], st.inv_sigma[HP - 1]);
         if (snr > best[u]) { best[u] = snr; bh[u] = HP; }
     }
 }
 
-// outputs e = 8 GRP + u of the lane: all levels
-template <int L, int W, int GRP>
+// outputs e = E0 + u, u < NE, of the lane: all levels
+template <int L, int W, int E0, int NE>
 __device__ __forceinline__ void level_chain(const float* __restrict__ sm, const HsStats& st, int w, int lane,
                                             float (&res_snr)[G], int (&res_bh)[G]) {
-    float S[8], best[8], add[8];
-    int bh[8];
-    add_terms<32, GRP, true>(row_ptr<0, W>(sm, w, lane), S);             // H' = 1: x[n]
+    float S[NE], best[NE], add[NE];
+    int bh[NE];
+    add_terms<32, E0, NE, true>(row_ptr<0, W>(sm, w, lane), S);             // H' = 1: x[n]
 #pragma unroll
-    for (int u = 0; u < 8; ++u) { best[u] = hs_snr(S[u], st.nmis[0], st.inv_sigma[0]); bh[u] = 1; }
+    for (int u = 0; u < NE; ++u) { best[u] = hs_snr(S[u], st.nmis[0], st.inv_sigma[0]); bh[u] = 1; }
     if (L >= 1) {
-        add_terms<16, GRP, true>(row_ptr<1, W>(sm, w, lane), add);
-        close_level<2>(st, S, add, best, bh);
+        add_terms<16, E0, NE, true>(row_ptr<1, W>(sm, w, lane), add);
+        close_level<2, NE>(st, S, add, best, bh);
     }
     if (L >= 2) {
-        add_terms<8, GRP, true>(row_ptr<2, W>(sm, w, lane), add);
-        close_level<4>(st, S, add, best, bh);
+        add_terms<8, E0, NE, true>(row_ptr<2, W>(sm, w, lane), add);
+        close_level<4, NE>(st, S, add, best, bh);
     }
     if (L >= 3) {
-        add_terms<4, GRP, true>(row_ptr<3, W>(sm, w, lane), add);
-        add_terms<24, GRP, false>(row_ptr<4, W>(sm, w, lane), add);
-        close_level<8>(st, S, add, best, bh);
+        add_terms<4, E0, NE, true>(row_ptr<3, W>(sm, w, lane), add);
+        add_terms<24, E0, NE, false>(row_ptr<4, W>(sm, w, lane), add);
+        close_level<8, NE>(st, S, add, best, bh);
     }
     if (L >= 4) {
-        add_terms<2, GRP, true>(row_ptr<5, W>(sm, w, lane), add);
-        add_terms<12, GRP, false>(row_ptr<6, W>(sm, w, lane), add);
-        add_terms<20, GRP, false>(row_ptr<7, W>(sm, w, lane), add);
-        add_terms<28, GRP, false>(row_ptr<8, W>(sm, w, lane), add);
-        close_level<16>(st, S, add, best, bh);
+        add_terms<2, E0, NE, true>(row_ptr<5, W>(sm, w, lane), add);
+        add_terms<12, E0, NE, false>(row_ptr<6, W>(sm, w, lane), add);
+        add_terms<20, E0, NE, false>(row_ptr<7, W>(sm, w, lane), add);
+        add_terms<28, E0, NE, false>(row_ptr<8, W>(sm, w, lane), add);
+        close_level<16, NE>(st, S, add, best, bh);
     }
     if (L >= 5) {
-        add_terms<1, GRP, true>(row_ptr<9, W>(sm, w, lane), add);
-        add_terms<6, GRP, false>(row_ptr<10, W>(sm, w, lane), add);
-        add_terms<10, GRP, false>(row_ptr<11, W>(sm, w, lane), add);
-        add_terms<14, GRP, false>(row_ptr<12, W>(sm, w, lane), add);
-        add_terms<18, GRP, false>(row_ptr<13, W>(sm, w, lane), add);
-        add_terms<22, GRP, false>(row_ptr<14, W>(sm, w, lane), add);
-        add_terms<26, GRP, false>(row_ptr<15, W>(sm, w, lane), add);
-        add_terms<30, GRP, false>(row_ptr<16, W>(sm, w, lane), add);
-        close_level<32>(st, S, add, best, bh);
+        add_terms<1, E0, NE, true>(row_ptr<9, W>(sm, w, lane), add);
+        add_terms<6, E0, NE, false>(row_ptr<10, W>(sm, w, lane), add);
+        add_terms<10, E0, NE, false>(row_ptr<11, W>(sm, w, lane), add);
+        add_terms<14, E0, NE, false>(row_ptr<12, W>(sm, w, lane), add);
+        add_terms<18, E0, NE, false>(row_ptr<13, W>(sm, w, lane), add);
+        add_terms<22, E0, NE, false>(row_ptr<14, W>(sm, w, lane), add);
+        add_terms<26, E0, NE, false>(row_ptr<15, W>(sm, w, lane), add);
+        add_terms<30, E0, NE, false>(row_ptr<16, W>(sm, w, lane), add);
+        close_level<32, NE>(st, S, add, best, bh);
     }
 #pragma unroll
-    for (int u = 0; u < 8; ++u) { res_snr[8 * GRP + u] = best[u]; res_bh[8 * GRP + u] = bh[u]; }
+    for (int u = 0; u < NE; ++u) { res_snr[E0 + u] = best[u]; res_bh[E0 + u] = bh[u]; }
 }
 
 }  // namespace hs_rows
 
-template <int L, int W, bool BULK>
-__global__ void __launch_bounds__(32 * W)
+// NE = 16 / 8: a warp does the 16 outputs of its lanes at once / as two groups of 8.
+// NE = -8 ("pair"): TWO warps share a 512-output tile, one takes outputs e < 8 of every lane's 16, the
+// other e >= 8: twice the warps for the same shared memory (the kernel's occupancy is set by shared memory).
+template <int L, int W, bool BULK, int NE>
+__global__ void __launch_bounds__(NE < 0 ? 64 * W : 32 * W, 12 / W)
 hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
     using namespace hs_rows;
-    constexpr int BLOCK = 32 * W;
+    constexpr bool PAIR = NE < 0;
+    constexpr int BLOCK = PAIR ? 64 * W : 32 * W;
     constexpr int T = WT * W;                           // outputs per CTA
     constexpr int NF = n_frac(L);
     extern __shared__ float4 hs_rows_smem4[];
@@ -273,29 +277,46 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 
     // ---- compute: lane i of warp w owns outputs n0 + 512 w + 16 i + [0, 16) ----
     const int lane = threadIdx.x & 31;
-    const int w = threadIdx.x >> 5;
+    const int w = PAIR ? (threadIdx.x >> 6) : (threadIdx.x >> 5);
+    const int half = PAIR ? ((threadIdx.x >> 5) & 1) : 0;
     float res_snr[G];
     int res_bh[G];
+    if (PAIR) {
+        if (half == 0) {
+            level_chain<L, W, 0, 8>(sm, st, w, lane, res_snr, res_bh);
+        } else {
+            level_chain<L, W, 8, 8>(sm, st, w, lane, res_snr, res_bh);
 #pragma unroll
-    for (int grp = 0; grp < 2; ++grp) {
-        if (grp == 0) level_chain<L, W, 0>(sm, st, w, lane, res_snr, res_bh);
-        else level_chain<L, W, 1>(sm, st, w, lane, res_snr, res_bh);
+            for (int u = 0; u < 8; ++u) { res_snr[u] = res_snr[8 + u]; res_bh[u] = res_bh[8 + u]; }   // registers 0..7 either way
+        }
+    } else if (NE == 16) {
+        level_chain<L, W, 0, 16>(sm, st, w, lane, res_snr, res_bh);
+    } else {
+        level_chain<L, W, 0, 8>(sm, st, w, lane, res_snr, res_bh);
+        level_chain<L, W, 8, 8>(sm, st, w, lane, res_snr, res_bh);
     }
 
-    // ---- store: transpose through the warp's own kk = 32 rows (32 rows x pitch 20, no longer read) ----
-    float* stg = sm + span_off(0, W) + 32 * w * pad_pitch(32);
+    // ---- store: transpose through the tile's own kk = 32 rows (32 rows x pitch 20, no longer read) ----
+    constexpr int P = pad_pitch(32);
+    float* stg = sm + span_off(0, W) + 32 * w * P;
+    int* stgi = reinterpret_cast<int*>(stg);
     const long long orow = (long long)s * sh.out_stride;
     const int nw = n0 + WT * w;
-    __syncwarp();
+    constexpr int V0 = 0, NV = PAIR ? 2 : 4;            // float4s of a row this warp writes / stream quarters it reads
+    const int vbase = PAIR ? 2 * half : V0;
+    auto sync_tile = [&]() { if (PAIR) __syncthreads(); else __syncwarp(); };
+    sync_tile();
 #pragma unroll
-    for (int v = 0; v < G / 4; ++v)
-        *reinterpret_cast<float4*>(stg + lane * pad_pitch(32) + 4 * v) =
+    for (int v = 0; v < NV; ++v) {
+        const int col = PAIR ? 8 * half + 4 * v : 4 * v;
+        *reinterpret_cast<float4*>(stg + lane * P + col) =
             make_float4(res_snr[4 * v], res_snr[4 * v + 1], res_snr[4 * v + 2], res_snr[4 * v + 3]);
-    __syncwarp();
+    }
+    sync_tile();
 #pragma unroll
-    for (int k = 0; k < G / 4; ++k) {
-        const int q = lane + 32 * k;                                  // float4 index in the warp's output stream
-        const float4 v = *reinterpret_cast<const float4*>(stg + (q >> 2) * pad_pitch(32) + 4 * (q & 3));
+    for (int k = 0; k < NV; ++k) {
+        const int q = lane + 32 * (vbase + k);                        // float4 index in the tile's output stream
+        const float4 v = *reinterpret_cast<const float4*>(stg + (q >> 2) * P + 4 * (q & 3));
         const int n = nw + 4 * q;
         if (n + 3 < n_fund) {
             __stcs(reinterpret_cast<float4*>(io.snr + orow + n), v);
@@ -305,17 +326,18 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             if (n + 2 < n_fund) st_cs(io.snr + orow + n + 2, v.z);
         }
     }
-    __syncwarp();
-    int* stgi = reinterpret_cast<int*>(stg);
+    sync_tile();
 #pragma unroll
-    for (int v = 0; v < G / 4; ++v)
-        *reinterpret_cast<int4*>(stgi + lane * pad_pitch(32) + 4 * v) =
+    for (int v = 0; v < NV; ++v) {
+        const int col = PAIR ? 8 * half + 4 * v : 4 * v;
+        *reinterpret_cast<int4*>(stgi + lane * P + col) =
             make_int4(res_bh[4 * v], res_bh[4 * v + 1], res_bh[4 * v + 2], res_bh[4 * v + 3]);
-    __syncwarp();
+    }
+    sync_tile();
 #pragma unroll
-    for (int k = 0; k < G / 4; ++k) {
-        const int q = lane + 32 * k;
-        const int4 v = *reinterpret_cast<const int4*>(stgi + (q >> 2) * pad_pitch(32) + 4 * (q & 3));
+    for (int k = 0; k < NV; ++k) {
+        const int q = lane + 32 * (vbase + k);
+        const int4 v = *reinterpret_cast<const int4*>(stgi + (q >> 2) * P + 4 * (q & 3));
         const int n = nw + 4 * q;
         if (n + 3 < n_fund) {
             __stcs(reinterpret_cast<int4*>(io.best_h + orow + n), v);
