@@ -40,7 +40,8 @@
  *   With d_inv_baseline != NULL every x[b] above is replaced by the fp32 product
  *   x[b] * inv_baseline[b] (spectrum whitening supplied by the caller).
  *   Sums are accumulated in fp32 in the order written above; the SNR is formed as
- *   (sum - mu) * (1/sigma) in fp32.  Non-finite inputs give unspecified results.
+ *   fma(sum, 1/sigma, -mu/sigma) in fp32, both constants rounded once on the host.  Non-finite
+ *   inputs give unspecified results.
  *
  * Memory, ownership, threading
  *   The caller owns every buffer.  d_* pointers are DEVICE pointers on the plan's device;
@@ -103,8 +104,9 @@ enum {
  *   n_fund     outputs are computed for n < n_fund (0 = n_bins); <= n_bins
  *   flags      OR of the enum above; HS_PRESTO_ALL_ORDERS requires HS_PRESTO_ALL_HARMONICS
  *   device     CUDA device ordinal
- * The plan owns only small internal state (device properties, launch geometry, and -- once
- * a *_host entry point has been used -- its staging buffers and streams). */
+ * The plan owns only small internal state (device properties, launch geometry, a comparison-mask
+ * scratch of one bit per bin for the few spectra the greedy mask variants keep in flight, and --
+ * once a *_host entry point has been used -- its staging buffers and streams). */
 hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
                   int64_t in_stride, int64_t out_stride, int64_t n_fund,
                   uint32_t flags, int32_t device);
