@@ -49,6 +49,10 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-spectra", type=int, default=64, help="spectra in the oracle's bounded sample")
+    ap.add_argument("--forms", default="both", choices=["both", "greedy", "presto"],
+                    help="which forms a step runs (cfg4 is quoted on the greedy form only)")
+    ap.add_argument("--greedy-flags", type=int, default=0, help="HS_GREEDY_* plan flags (NEXT-1 variants)")
+    ap.add_argument("--presto-flags", type=int, default=0, help="HS_PRESTO_* plan flags (NEXT-1 variants)")
     ap.add_argument("--tune-greedy", type=int, default=0)
     ap.add_argument("--tune-presto", type=int, default=0)
     return ap.parse_args()
@@ -138,18 +142,31 @@ def barrier(world):
     torch.cuda.synchronize()
 
 
-def run_cpu_sample(x_host, H, n_threads=None):
+def _variants(args):
+    """(greedy stats variant, fund_select, PRESTO stats variant) for the plan flags of this run."""
+    gv = "simple" if args.greedy_flags & 2 else "greedy"
+    pv = "presto_plus" if (args.presto_flags & 12) == 12 else "presto_all" if args.presto_flags & 4 else "presto"
+    return gv, not (args.greedy_flags & 1), pv
+
+
+def run_cpu_sample(x_host, H, n_threads=None, args=None, ib_host=None):
     """Time the oracle, as it stands, on a [rows, N] float32 numpy sample: greedy then PRESTO."""
     import oracle
     from paper_2202_12817_b200 import inputs
     oracle.build()
     cores = n_threads or oracle.host_threads()
-    mu_g, sg_g = inputs.exp1_stats("greedy", H)
-    mu_p, sg_p = inputs.exp1_stats("presto", H)
+    gv, fs, pv = _variants(args) if args is not None else ("greedy", True, "presto")
+    gflags = args.greedy_flags if args is not None else 0
+    pflags = args.presto_flags if args is not None else 0
+    forms = args.forms if args is not None else "both"
+    mu_g, sg_g = inputs.exp1_stats(gv, H, fs)
+    mu_p, sg_p = inputs.exp1_stats(pv, H)
     t0 = time.perf_counter()
-    oracle.greedy(x_host, H, mu_g.numpy(), sg_g.numpy(), n_threads=cores, want_path=False)
+    if forms != "presto":
+        oracle.greedy(x_host, H, mu_g.numpy(), sg_g.numpy(), gflags, inv_baseline=ib_host, n_threads=cores, want_path=False)
     t1 = time.perf_counter()
-    oracle.presto(x_host, H, mu_p.numpy(), sg_p.numpy(), n_threads=cores)
+    if forms != "greedy":
+        oracle.presto(x_host, H, mu_p.numpy(), sg_p.numpy(), pflags, inv_baseline=ib_host, n_threads=cores)
     t2 = time.perf_counter()
     bins = x_host.shape[0] * x_host.shape[1]
     return {"bins": bins, "seconds": t2 - t0, "greedy_s": t1 - t0, "presto_s": t2 - t1, "cores": cores}
@@ -203,23 +220,33 @@ def run_cuda(args):
     x = torch.empty((S, N), dtype=torch.float32, device=dev)
     for s in range(S):
         x[s].copy_(inputs.generate_row(w, rank * S + s, dev))
+    do_g, do_p = args.forms != "presto", args.forms != "greedy"
+    # cfg4: the caller's whitening estimate, a per-bin reciprocal block-median baseline (NEXT-2)
+    ib = None
+    if w.red_noise:
+        ib = torch.empty((S, N), dtype=torch.float32, device=dev)
+        for s in range(S):
+            ib[s:s + 1].copy_(inputs.block_median_inv_baseline(x[s:s + 1]))
     snr_g = torch.empty((S, N), dtype=torch.float32, device=dev)
     bh_g = torch.empty((S, N), dtype=torch.int32, device=dev)
-    snr_p = torch.empty_like(snr_g)
-    bh_p = torch.empty_like(bh_g)
-    mu_g, sg_g = inputs.exp1_stats("greedy", H)
-    mu_p, sg_p = inputs.exp1_stats("presto", H)
-    plan_g = hs.hs_plan(N, S, H, flags=args.tune_greedy << hs.HS_TUNE_SHIFT, device=local)
-    plan_p = hs.hs_plan(N, S, H, flags=args.tune_presto << hs.HS_TUNE_SHIFT, device=local)
+    snr_p = torch.empty_like(snr_g) if do_p and do_g else snr_g
+    bh_p = torch.empty_like(bh_g) if do_p and do_g else bh_g
+    gv, fs, pv = _variants(args)
+    mu_g, sg_g = inputs.exp1_stats(gv, H, fs)
+    mu_p, sg_p = inputs.exp1_stats(pv, H)
+    plan_g = hs.hs_plan(N, S, H, flags=args.greedy_flags | (args.tune_greedy << hs.HS_TUNE_SHIFT), device=local)
+    plan_p = hs.hs_plan(N, S, H, flags=args.presto_flags | (args.tune_presto << hs.HS_TUNE_SHIFT), device=local)
     stream = torch.cuda.current_stream(dev)
 
     def step(ev=None):
         if ev is not None:
             ev[0].record(stream)
-        hs.hs_run_greedy(plan_g, x, None, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
+        if do_g:
+            hs.hs_run_greedy(plan_g, x, ib, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
         if ev is not None:
             ev[1].record(stream)
-        hs.hs_run_presto(plan_p, x, None, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
+        if do_p:
+            hs.hs_run_presto(plan_p, x, ib, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
         if ev is not None:
             ev[2].record(stream)
 
@@ -252,6 +279,9 @@ def run_cuda(args):
     g_ms = max_over_ranks(g_ms, dev)
     p_ms = max_over_ranks(p_ms, dev)
     bins_step = float(S) * N * world
+    n_forms = int(do_g) + int(do_p)
+    default_run = (args.forms == "both" and not args.greedy_flags and not args.presto_flags and ib is None
+                   and not args.tune_greedy and not args.tune_presto and w.name == "cfg3" and S == w.n_spectra)
     value = bins_step * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the host-buffer entry points (pinned host memory, H2D + D2H timed) ----
@@ -263,9 +293,16 @@ def run_cuda(args):
         hbh = torch.empty((S, N), dtype=torch.int32, pin_memory=True)
         e_steps = max(1, min(args.steps, 5))
 
+        hib = None
+        if ib is not None:
+            hib = torch.empty((S, N), dtype=torch.float32, pin_memory=True)
+            hib.copy_(ib)
+
         def e2e_step():
-            hs.hs_run_greedy_host(plan_g, hx, None, mu_g, sg_g, hsnr, hbh, None)
-            hs.hs_run_presto_host(plan_p, hx, None, mu_p, sg_p, hsnr, hbh)
+            if do_g:
+                hs.hs_run_greedy_host(plan_g, hx, hib, mu_g, sg_g, hsnr, hbh, None)
+            if do_p:
+                hs.hs_run_presto_host(plan_p, hx, hib, mu_p, sg_p, hsnr, hbh)
 
         e2e_step()
         barrier(world)
@@ -275,15 +312,16 @@ def run_cuda(args):
         barrier(world)
         dt = max_over_ranks(time.perf_counter() - t0, dev)
         e2e = {"value": bins_step * e_steps / dt, "unit": UNIT, "steps": e_steps,
-               "h2d_bytes_per_step": 2 * S * N * 4, "d2h_bytes_per_step": 2 * S * N * 8,
+               "h2d_bytes_per_step": n_forms * S * N * 4 * (2 if ib is not None else 1),
+               "d2h_bytes_per_step": n_forms * S * N * 8,
                "ms_per_step": 1e3 * dt / e_steps,
                "note": "hs_run_greedy_host + hs_run_presto_host, pinned host buffers, per rank; PCIe-bound"}
-        del hx, hsnr, hbh
+        del hx, hsnr, hbh, hib
 
     # ---- roofline of the dominant kernel (HBM-bound: 12 algorithmic bytes per bin and launch) ----
     peak, peak_src = measured_peak()
-    dom, dom_ms = ("greedy", g_ms) if g_ms >= p_ms else ("presto", p_ms)
-    alg_bytes = BYTES_PER_BIN * S * N
+    dom, dom_ms = ("greedy", g_ms) if (g_ms >= p_ms or not do_p) and do_g else ("presto", p_ms)
+    alg_bytes = (BYTES_PER_BIN + (4.0 if ib is not None else 0.0)) * S * N
 
     def roof(ms):
         a = alg_bytes / (ms * 1e-3) / 1e9
@@ -291,17 +329,20 @@ def run_cuda(args):
 
     a, fr = roof(dom_ms)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": a, "peak": peak, "unit": "GB/s", "frac": fr,
-                "traffic": NCU_TRAFFIC_BYTES[dom], "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_BYTES[dom] if default_run else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": dom_ms,
-                "per_kernel": {"greedy": {"launch_ms": g_ms, "achieved": roof(g_ms)[0], "frac": roof(g_ms)[1],
-                                          "gbins_per_s": S * N / g_ms / 1e6},
-                               "presto": {"launch_ms": p_ms, "achieved": roof(p_ms)[0], "frac": roof(p_ms)[1],
-                                          "gbins_per_s": S * N / p_ms / 1e6}}}
+                "per_kernel": {}}
+    if do_g:
+        roofline["per_kernel"]["greedy"] = {"launch_ms": g_ms, "achieved": roof(g_ms)[0], "frac": roof(g_ms)[1],
+                                            "gbins_per_s": S * N / g_ms / 1e6}
+    if do_p:
+        roofline["per_kernel"]["presto"] = {"launch_ms": p_ms, "achieved": roof(p_ms)[0], "frac": roof(p_ms)[1],
+                                            "gbins_per_s": S * N / p_ms / 1e6}
 
     cpu = None
     if rank == 0 and not args.no_cpu:
         rows = min(args.cpu_spectra, S)
-        r = run_cpu_sample(x[:rows].cpu().numpy(), H)
+        r = run_cpu_sample(x[:rows].cpu().numpy(), H, args=args, ib_host=None if ib is None else ib[:rows].cpu().numpy())
         cpu = {"value": r["bins"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                "sample": f"first {rows} of {S} spectra of {w.name} ({rows}x{N} bins), greedy {r['greedy_s']:.2f} s + "
                          f"PRESTO {r['presto_s']:.2f} s, fp64"}
@@ -311,8 +352,12 @@ def run_cuda(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": f"{w.name}: {S} spectra x {N} fp32 bins per GPU, H={H}, greedy (Alg. 2) + PRESTO (Alg. 1) per step",
-                           "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": "inputs (4 GiB) exceed L2; no flush needed",
+                "config": {"workload": f"{w.name}: {S} spectra x {N} fp32 bins per GPU, H={H}, " +
+                                       {"both": "greedy (Alg. 2) + PRESTO (Alg. 1) per step", "greedy": "greedy (Alg. 2) only",
+                                        "presto": "PRESTO (Alg. 1) only"}[args.forms] +
+                                       (f", stats/flags {gv}/{pv} ({args.greedy_flags}/{args.presto_flags})" if args.greedy_flags or args.presto_flags else "") +
+                                       (", per-bin inverse baseline" if ib is not None else ""),
+                           "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "cpu_baseline": cpu}

@@ -93,7 +93,12 @@ hs_status launch_greedy_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     dim3 grid((unsigned)((sh.n_fund + tile - 1) / tile), (unsigned)sh.n_spectra);
     const bool fs = !(sh.flags & HS_GREEDY_NO_FUND_SELECT);
     const bool wp = io.path != nullptr;
-    if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    if (io.inv_base) {
+        if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+        else if (fs && !wp) hs_greedy_tile_kernel<BLOCK, R, true, false, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+        else if (!fs && wp) hs_greedy_tile_kernel<BLOCK, R, false, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+        else hs_greedy_tile_kernel<BLOCK, R, false, false, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    } else if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
     else if (fs && !wp) hs_greedy_tile_kernel<BLOCK, R, true, false><<<grid, BLOCK, 0, stream>>>(sh, st, io);
     else if (!fs && wp) hs_greedy_tile_kernel<BLOCK, R, false, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
     else hs_greedy_tile_kernel<BLOCK, R, false, false><<<grid, BLOCK, 0, stream>>>(sh, st, io);
@@ -151,8 +156,8 @@ hs_status launch_greedy_band(hs_plan_s* p, const HsShape& full, const HsStats& s
 hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
-    const bool fast_ok = !io.inv_base && !(sh.flags & HS_GREEDY_NO_DRIFT) && sh.n_bins <= (1ll << 31) - 64 && p->tune != 255;
-    if (fast_ok && p->d_mask && sh.n_bins <= (1ll << 30)) {
+    const bool fast_ok = !(sh.flags & HS_GREEDY_NO_DRIFT) && sh.n_bins <= (1ll << 31) - 64 && p->tune != 255;
+    if (fast_ok && !io.inv_base && p->d_mask && sh.n_bins <= (1ll << 30)) {
         switch (p->tune) {
             case 20: return launch_greedy_band<256, 1, 2>(p, sh, st, io, stream);
             case 21: return launch_greedy_band<256, 2, 2>(p, sh, st, io, stream);

@@ -12,7 +12,8 @@
 #pragma once
 #include "hs_common.cuh"
 
-template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH>
+// HAS_BASE: every x[b] is the fp32 product x[b] * inv_baseline[b] (reading R13; cfg4's whitening multiplier).
+template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false>
 __global__ void __launch_bounds__(BLOCK)
 hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
     const int s = blockIdx.y;
@@ -21,6 +22,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int n_fund = (int)sh.n_fund;
     const int f0 = blockIdx.x * (BLOCK * R);
     const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
+    const float* __restrict__ ib = HAS_BASE ? io.inv_base + (long long)s * sh.in_stride : nullptr;
 
     // Orders 1..h_safe need no band-edge test for any fundamental of the tile:
     // m + 1 = h n + d + 1 <= h (n + 1) + 1 <= last.   Orders above h_top are dead for all of them.
@@ -55,6 +57,10 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             const int m = hn[j] + d[j];
             a[j] = __ldg(x + m);
             b[j] = __ldg(x + m + 1);
+            if (HAS_BASE) {
+                a[j] = __fmul_rn(a[j], __ldg(ib + m));
+                b[j] = __fmul_rn(b[j], __ldg(ib + m + 1));
+            }
         }
 #pragma unroll
         for (int j = 0; j < R; ++j) {
@@ -79,9 +85,13 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             const int m = hn[j] + d[j];
             alive[j] = alive[j] && (m <= last);
             if (alive[j]) {
-                const float a = __ldg(x + m);
+                float a = __ldg(x + m);
+                if (HAS_BASE) a = __fmul_rn(a, __ldg(ib + m));
                 float b = HS_NEG_INF;
-                if (m + 1 <= last && (FUND_SELECT || h != 1)) b = __ldg(x + m + 1);
+                if (m + 1 <= last && (FUND_SELECT || h != 1)) {
+                    b = __ldg(x + m + 1);
+                    if (HAS_BASE) b = __fmul_rn(b, __ldg(ib + m + 1));
+                }
                 const bool shift = b > a;
                 d[j] += shift;
                 sum[j] = __fadd_rn(sum[j], shift ? b : a);

@@ -217,12 +217,30 @@ def test_inv_baseline_red_noise(hs, oracle_mod):
     xt = inputs.generate(w)
     ib = inputs.block_median_inv_baseline(xt).numpy()
     x = xt.numpy()
-    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
-    s, b, p = run_greedy(hs, x, H, mu, sg, 0, inv_baseline=ib)
-    check_greedy(oracle_mod, x, H, mu, sg, 0, s, b, p, inv_baseline=ib, T=10.0)
+    for tune in (0, 3, 255):                 # tuned tile kernels with the multiplier, and the generic kernel
+        for flags, fs in ((0, True), (NO_FUND_SELECT, False)):
+            mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H, fs))
+            s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16), inv_baseline=ib)
+            check_greedy(oracle_mod, x, H, mu, sg, flags, s, b, p, inv_baseline=ib, T=10.0)
     mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
     s, b = run_presto(hs, x, H, mu, sg, 0, inv_baseline=ib)
     check_presto(oracle_mod, x, H, mu, sg, 0, s, b, inv_baseline=ib, T=10.0)
+
+
+@pytest.mark.parametrize("tune", [0, 1, 6, 255])
+def test_inv_baseline_exact_integer(hs, oracle_mod, tune):
+    """Integer powers times power-of-two multipliers: every product, sum and SNR is exact (pin P7 with R13)."""
+    H = 32
+    mu, sg = _int_stats(H)
+    S, N = 3, 30011
+    x = inputs.integer_spectra(31, S, N, 63).numpy()
+    rng = np.random.default_rng(5)
+    ib = (2.0 ** rng.integers(-1, 3, size=(S, N))).astype(np.float32)
+    for flags in (0, NO_FUND_SELECT):
+        s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags, inv_baseline=ib)
+        s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16), inv_baseline=ib)
+        assert np.array_equal(p.view(np.uint32), p_ref) and np.array_equal(b, b_ref)
+        assert np.array_equal(s.astype(np.float64), s_ref)
 
 
 # ------------------------------------------------------------------------------------------
