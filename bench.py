@@ -318,6 +318,23 @@ def run_cuda(args):
                "note": "hs_run_greedy_host + hs_run_presto_host, pinned host buffers, per rank; PCIe-bound"}
         del hx, hsnr, hbh, hib
 
+    # ---- NEXT-3: candidate list of the greedy outputs (one streaming pass; outside the step) ----
+    cand = None
+    if do_g:
+        T = 10.0
+        cbuf = torch.empty((1 << 20, 4), dtype=torch.int32, device=dev)
+        ccnt = torch.zeros((1,), dtype=torch.int64, device=dev)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        hs.hs_find_candidates(plan_g, snr_g, bh_g, T, cbuf, ccnt, stream.cuda_stream)
+        c0.record(stream)
+        for _ in range(5):
+            hs.hs_find_candidates(plan_g, snr_g, bh_g, T, cbuf, ccnt, stream.cuda_stream)
+        c1.record(stream)
+        torch.cuda.synchronize()
+        c_ms = c0.elapsed_time(c1) / 5
+        cand = {"threshold": T, "count": int(ccnt.item()), "ms": c_ms, "read_gbs": S * N * 4 / (c_ms * 1e-3) / 1e9}
+        del cbuf
+
     # ---- roofline of the dominant kernel (HBM-bound: 12 algorithmic bytes per bin and launch) ----
     peak, peak_src = measured_peak()
     dom, dom_ms = ("greedy", g_ms) if (g_ms >= p_ms or not do_p) and do_g else ("presto", p_ms)
@@ -359,7 +376,7 @@ def run_cuda(args):
                                        (", per-bin inverse baseline" if ib is not None else ""),
                            "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "candidates": cand,
                 "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -140,6 +140,24 @@ hs_status hs_run_presto_host(hs_plan_t plan, const float* h_spectra, const float
                              const float* mu, const float* sigma,
                              float* h_snr, int32_t* h_best_h);
 
+/* One detection (reading R11 of DESIGN.md: a bin whose maximum SNR reaches the threshold). */
+typedef struct {
+    int32_t spectrum;   /* row s of the batch */
+    int32_t bin;        /* n (greedy: the fundamental bin; PRESTO: the top bin) */
+    float   snr;        /* d_snr[s][n] */
+    int32_t best_h;     /* d_best_h[s][n] */
+} hs_candidate;
+
+/* Candidate list of a finished run: every (s, n), n < n_fund, with d_snr[s][n] >= threshold (NaN never
+ * qualifies), in unspecified order (sort by (spectrum, bin) for a canonical list).
+ *   d_snr, d_best_h  outputs of hs_run_greedy / hs_run_presto of the same plan (device, [S][out_stride])
+ *   d_out            device array of `capacity` hs_candidate (16-byte aligned); may be NULL if capacity = 0
+ *   d_count          device uint64: set to the number of qualifying bins, which may exceed `capacity`
+ *                    (then only `capacity` of them were stored: call again with a larger array)
+ * Asynchronous on the stream; one streaming pass over d_snr. */
+hs_status hs_find_candidates(hs_plan_t plan, const float* d_snr, const int32_t* d_best_h, float threshold,
+                             hs_candidate* d_out, int64_t capacity, uint64_t* d_count, void* cuda_stream);
+
 /* Number of kernels this plan has launched so far (for bench.py's gpu_launches). */
 int64_t hs_launch_count(hs_plan_t plan);
 

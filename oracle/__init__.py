@@ -197,3 +197,11 @@ def presto_orders(H: int, flags: int = 0):
     """ORDERS(H): the H' values Alg. 1's outer loop visits."""
     lib = _load()
     return [Hp for Hp in range(1, H + 1) if lib.hs_oracle_presto_order_in_set(Hp, flags)]
+
+
+def candidates(snr, best_h, threshold: float):
+    """Reading R11: every (spectrum, bin) with snr >= threshold, with its best_h, sorted by
+    (spectrum, bin).  Returns an int64 array [k, 3] (spectrum, bin, best_h) and the float64 snr values [k]."""
+    snr = np.asarray(snr)
+    rows, bins = np.nonzero(snr >= threshold)          # row-major order = sorted by (spectrum, bin); NaN never qualifies
+    return np.stack([rows, bins, np.asarray(best_h)[rows, bins]], axis=1).astype(np.int64), snr[rows, bins].astype(np.float64)

@@ -24,7 +24,7 @@ HS_PRESTO_ALL_HARMONICS = 1 << 2
 HS_PRESTO_ALL_ORDERS = 1 << 3
 HS_TUNE_SHIFT = 16
 
-EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host",
+EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_find_candidates",
            "hs_launch_count", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -61,6 +61,8 @@ def load() -> ctypes.CDLL:
     lib.hs_run_greedy_host.restype = ctypes.c_int
     lib.hs_run_presto_host.argtypes = [vp, vp, vp, fp, fp, vp, vp]
     lib.hs_run_presto_host.restype = ctypes.c_int
+    lib.hs_find_candidates.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp, vp]
+    lib.hs_find_candidates.restype = ctypes.c_int
     lib.hs_launch_count.argtypes = [vp]
     lib.hs_launch_count.restype = i64
     lib.hs_destroy.argtypes = [vp]
@@ -147,6 +149,21 @@ def hs_run_presto_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best
                                   _hptr(h_inv_baseline, torch.float32, "h_inv_baseline"), _farr(mu), _farr(sigma),
                                   _hptr(h_snr, torch.float32, "h_snr"), _hptr(h_best_h, torch.int32, "h_best_h")),
            "hs_run_presto_host")
+
+
+def hs_find_candidates(plan, d_snr: torch.Tensor, d_best_h: torch.Tensor, threshold: float,
+                       d_out: Optional[torch.Tensor], d_count: torch.Tensor, stream: Optional[int] = None) -> None:
+    """d_out: int32 CUDA tensor [capacity, 4] (rows = hs_candidate: spectrum, bin, snr bits, best_h) or None;
+    d_count: int64 CUDA tensor with one element (uint64 count)."""
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_snr.device).cuda_stream
+    cap = 0 if d_out is None else int(d_out.shape[0])
+    if d_out is not None and (d_out.ndim != 2 or d_out.shape[1] != 4):
+        raise TypeError("d_out: expected an int32 tensor of shape [capacity, 4]")
+    _check(lib.hs_find_candidates(plan, _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                                  float(threshold), _dptr(d_out, torch.int32, "d_out"), cap,
+                                  _dptr(d_count, torch.int64, "d_count"), stream), "hs_find_candidates")
 
 
 def hs_launch_count(plan) -> int:

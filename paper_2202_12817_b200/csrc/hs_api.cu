@@ -16,6 +16,7 @@
 #include "hs_presto_smem.cuh"
 #include "hs_presto_rows.cuh"
 #include "hs_presto_pipe.cuh"
+#include "hs_candidates.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -520,6 +521,30 @@ hs_status hs_run_greedy_host(hs_plan_t plan, const float* h_spectra, const float
 hs_status hs_run_presto_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline, const float* mu,
                              const float* sigma, float* h_snr, int32_t* h_best_h) {
     return run_host(plan, false, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best_h, nullptr);
+}
+
+hs_status hs_find_candidates(hs_plan_t plan, const float* d_snr, const int32_t* d_best_h, float threshold,
+                             hs_candidate* d_out, int64_t capacity, uint64_t* d_count, void* cuda_stream) {
+    static_assert(sizeof(hs_candidate) == sizeof(HsCandidate) && sizeof(hs_candidate) == 16, "candidate layout");
+    if (!plan || !d_snr || !d_best_h || !d_count || capacity < 0 || (capacity > 0 && !d_out)) return HS_ERR_INVALID_ARG;
+    if (!aligned16(d_snr) || !aligned16(d_best_h) || (d_out && !aligned16(d_out)) || (reinterpret_cast<uintptr_t>(d_count) & 7u))
+        return HS_ERR_INVALID_ARG;
+    if (!(threshold == threshold)) return HS_ERR_INVALID_ARG;
+    const HsShape& sh = plan->shape;
+    if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    HS_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint64_t), stream));
+    if (sh.n_fund == 0) return HS_OK;
+    const long long n4 = (sh.n_fund + 3) / 4;
+    // a few waves of 256-thread CTAs per spectrum row, grid-stride inside the row
+    const long long per_row = std::max(1ll, std::min((n4 + 255) / 256, (long long)std::max(1, plan->sm_count * 64 / sh.n_spectra + 1)));
+    dim3 grid((unsigned)per_row, (unsigned)sh.n_spectra);
+    hs_candidates_kernel<256><<<grid, 256, 0, stream>>>(d_snr, d_best_h, sh.out_stride, (int)sh.n_fund, threshold,
+                                                        reinterpret_cast<HsCandidate*>(d_out), (unsigned long long)capacity,
+                                                        reinterpret_cast<unsigned long long*>(d_count));
+    plan->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
 }
 
 int64_t hs_launch_count(hs_plan_t plan) { return plan ? plan->launches : -1; }

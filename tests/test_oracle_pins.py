@@ -414,3 +414,15 @@ def test_argument_validation(oracle_mod):
         oracle_mod.presto(x, 2, [1, 2], [1, 1], ALL_ORDERS)  # ALL_ORDERS needs ALL_HARMONICS
     with pytest.raises(ValueError):
         oracle_mod.greedy(x, 33, np.ones(33), np.ones(33))
+
+
+def test_candidates_definition_brute_force():
+    """R11: the candidate list is the plain threshold definition; pinned by a Python loop on a tiny array
+    (ties at the threshold count, NaN does not)."""
+    import oracle
+    snr = np.array([[1.0, 10.0, np.nan, 12.5], [9.999, 10.0001, -3.0, 1e9]], np.float32)
+    bh = np.array([[1, 2, 3, 4], [5, 6, 7, 8]], np.int32)
+    want = [(s, n, int(bh[s, n])) for s in range(2) for n in range(4) if float(snr[s, n]) >= 10.0]
+    got, vals = oracle.candidates(snr, bh, 10.0)
+    assert [tuple(r) for r in got.tolist()] == want == [(0, 1, 2), (0, 3, 4), (1, 1, 6), (1, 3, 8)]
+    assert vals.tolist() == [float(snr[s, n]) for s, n, _ in want]

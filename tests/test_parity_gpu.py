@@ -243,6 +243,80 @@ def test_inv_baseline_exact_integer(hs, oracle_mod, tune):
         assert np.array_equal(s.astype(np.float64), s_ref)
 
 
+def _gpu_candidates(hs, plan, snr, bh, T, capacity):
+    out = torch.full((max(capacity, 1), 4), -1, dtype=torch.int32, device="cuda")
+    cnt = torch.full((1,), -5, dtype=torch.int64, device="cuda")
+    hs.hs_find_candidates(plan, snr, bh, T, out if capacity else None, cnt)
+    torch.cuda.synchronize()
+    k = int(cnt.item())
+    got = out[:min(k, capacity)].cpu().numpy()
+    order = np.lexsort((got[:, 1], got[:, 0]))
+    return k, got[order]
+
+
+def test_candidates_list(hs, oracle_mod):
+    """NEXT-3 / north_star check (c): the candidate list produced on the GPU.  Exact against the plain definition
+    applied to the same GPU outputs (integer / selection work), and equal to the oracle's list away from the threshold."""
+    w = inputs.workload("cfg1")
+    H, T = w.H, 10.0
+    x = inputs.generate(w)
+    S, N = x.shape
+    mu, sg = inputs.exp1_stats("greedy", H)
+    dx = x.cuda()
+    for n_fund, ostr in ((0, 0), (50001, 50004)):
+        nf = n_fund or N
+        ostride = ostr or N
+        snr = torch.empty((S, ostride), dtype=torch.float32, device="cuda")
+        bh = torch.empty((S, ostride), dtype=torch.int32, device="cuda")
+        plan = hs.hs_plan(N, S, H, 0, ostride, n_fund, 0, 0)
+        try:
+            hs.hs_run_greedy(plan, dx, None, mu, sg, snr, bh, None)
+            snr[:, nf:] = 1e9                                       # nothing outside [0, n_fund) may be reported
+            k, got = _gpu_candidates(hs, plan, snr, bh, T, 1 << 16)
+            ref, ref_snr = oracle_mod.candidates(snr[:, :nf].cpu().numpy(), bh[:, :nf].cpu().numpy(), T)
+            assert k == ref.shape[0] > 0
+            assert np.array_equal(got[:, [0, 1, 3]].astype(np.int64), ref)
+            assert np.array_equal(got[:, 2].copy().view(np.float32).astype(np.float64), ref_snr)
+            # against the oracle's own outputs: equal except bins whose oracle snr is within tol of T
+            s_ref, b_ref, _ = oracle_mod.greedy(x.numpy(), H, mu.numpy(), sg.numpy(), 0, n_fund=nf)
+            oref, _ = oracle_mod.candidates(s_ref, b_ref, T)
+            near = {(r, c) for r, c in zip(*np.nonzero(np.abs(s_ref - T) <= 2e-5 * max(1.0, T)))}
+            a = {(int(r), int(c)) for r, c, _ in ref} - near
+            b = {(int(r), int(c)) for r, c, _ in oref} - near
+            assert a == b
+            # capacity smaller than the list: the count is still the full count, nothing is written past capacity
+            k2, got2 = _gpu_candidates(hs, plan, snr, bh, T, 3)
+            assert k2 == k and got2.shape[0] == 3
+            k3, _ = _gpu_candidates(hs, plan, snr, bh, T, 0)
+            assert k3 == k
+            k4, got4 = _gpu_candidates(hs, plan, snr, bh, 1e30, 8)
+            assert k4 == 0 and got4.shape[0] == 0
+        finally:
+            hs.hs_destroy(plan)
+
+
+def test_candidates_dense_and_batch(hs, oracle_mod):
+    """Every bin a hit (threshold -inf) and a ragged multi-spectrum batch: count and content exact."""
+    S, N, H = 5, 70001, 8
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(77, S, N, 255)
+    snr = torch.empty((S, N + 3), dtype=torch.float32, device="cuda")
+    bh = torch.empty((S, N + 3), dtype=torch.int32, device="cuda")
+    dx = torch.zeros((S, N + 3), dtype=torch.float32, device="cuda")
+    dx[:, :N] = x.cuda()
+    plan = hs.hs_plan(N, S, H, N + 3, N + 3, 0, 0, 0)
+    try:
+        hs.hs_run_presto(plan, dx, None, mu, sg, snr, bh)
+        for T in (-1e30, 40.0):
+            k, got = _gpu_candidates(hs, plan, snr, bh, T, S * N)
+            ref, ref_snr = oracle_mod.candidates(snr[:, :N].cpu().numpy(), bh[:, :N].cpu().numpy(), T)
+            assert k == ref.shape[0]
+            assert np.array_equal(got[:, [0, 1, 3]].astype(np.int64), ref)
+            assert np.array_equal(got[:, 2].copy().view(np.float32).astype(np.float64), ref_snr)
+    finally:
+        hs.hs_destroy(plan)
+
+
 # ------------------------------------------------------------------------------------------
 # Host-buffer entry points (the e2e leg of bench.py) and error behaviour
 # ------------------------------------------------------------------------------------------
