@@ -183,7 +183,7 @@ hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 6: return launch_greedy_tile<128, 4>(p, sh, st, io, stream);
             case 7: return launch_greedy_tile<512, 1>(p, sh, st, io, stream);
             case 8: return launch_greedy_tile<512, 2>(p, sh, st, io, stream);
-            default: return launch_greedy_tile<256, 2>(p, sh, st, io, stream);
+            default: return launch_greedy_tile<256, 4>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);

@@ -32,6 +32,31 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     h_safe = min(h_safe, H);
     const int h_top = (f0 == 0) ? H : min(H, last / f0);
 
+    // ---- top band: order 1 is the only order of every fundamental of the tile (2 f0 > N - 1): pure streaming.
+    // A thread takes 4 consecutive bins: one 16-byte load, the neighbour's first word by shuffle, 16-byte stores.
+    if (!HAS_BASE && h_top == 1 && f0 + BLOCK * R <= n_fund && f0 + BLOCK * R + 1 <= N && (BLOCK * R) % 128 == 0) {
+        if (threadIdx.x < BLOCK * R / 4) {                          // whole warps: BLOCK R / 4 is a multiple of 32
+            const int n0 = f0 + 4 * threadIdx.x;
+            const float4 v = __ldg(reinterpret_cast<const float4*>(x + n0));
+            float nxt = __shfl_down_sync(0xffffffffu, v.x, 1);
+            if ((threadIdx.x & 31) == 31) nxt = __ldg(x + n0 + 4);
+            const float e[5] = {v.x, v.y, v.z, v.w, nxt};
+            float snr[4];
+            unsigned pb[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const bool shift = FUND_SELECT && e[k + 1] > e[k];  // strict >: ties stay
+                snr[k] = hs_snr(shift ? e[k + 1] : e[k], st.nmis[0], st.inv_sigma[0]);
+                pb[k] = shift ? 1u : 0u;
+            }
+            const long long o = (long long)s * sh.out_stride + n0;
+            __stcs(reinterpret_cast<float4*>(io.snr + o), make_float4(snr[0], snr[1], snr[2], snr[3]));
+            __stcs(reinterpret_cast<int4*>(io.best_h + o), make_int4(1, 1, 1, 1));
+            if (WANT_PATH) __stcs(reinterpret_cast<uint4*>(io.path + o), make_uint4(pb[0], pb[1], pb[2], pb[3]));
+        }
+        return;
+    }
+
     int n[R], d[R], hn[R], bh[R];
     float sum[R], best[R];
     unsigned path[R];
