@@ -15,7 +15,6 @@
 #include "hs_presto.cuh"
 #include "hs_presto_smem.cuh"
 #include "hs_presto_rows.cuh"
-#include "hs_presto_pipe.cuh"
 #include "hs_candidates.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
@@ -266,39 +265,6 @@ hs_status launch_presto_rows(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     }
 }
 
-template <int L, int NWARP>
-hs_status launch_presto_pipe_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
-    constexpr int smem = 4 * NWARP * hs_rows::smem_words(L, 1);
-    static int ctas_per_sm = 0;                         // per instantiation
-    if (!ctas_per_sm) {
-        HS_CUDA(cudaFuncSetAttribute(hs_presto_pipe_kernel<L, NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        int nb = 0;
-        HS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, hs_presto_pipe_kernel<L, NWARP>, 32 * NWARP, smem));
-        ctas_per_sm = std::max(1, nb);
-    }
-    const long long tiles_per_row = (sh.n_fund + 511) / 512;
-    const long long total = tiles_per_row * sh.n_spectra;
-    if (total > 0x7fffffffll) return HS_ERR_UNSUPPORTED;
-    const long long want = (total + NWARP - 1) / NWARP;
-    const unsigned grid = (unsigned)std::min<long long>(want, (long long)p->sm_count * ctas_per_sm);
-    hs_presto_pipe_kernel<L, NWARP><<<grid, 32 * NWARP, smem, stream>>>(sh, st, io, (int)tiles_per_row, (int)total);
-    p->launches += 1;
-    HS_CUDA(cudaGetLastError());
-    return HS_OK;
-}
-
-template <int NWARP>
-hs_status launch_presto_pipe(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
-    switch (floor_log2(sh.H)) {
-        case 0: return launch_presto_pipe_L<0, NWARP>(p, sh, st, io, stream);
-        case 1: return launch_presto_pipe_L<1, NWARP>(p, sh, st, io, stream);
-        case 2: return launch_presto_pipe_L<2, NWARP>(p, sh, st, io, stream);
-        case 3: return launch_presto_pipe_L<3, NWARP>(p, sh, st, io, stream);
-        case 4: return launch_presto_pipe_L<4, NWARP>(p, sh, st, io, stream);
-        default: return launch_presto_pipe_L<5, NWARP>(p, sh, st, io, stream);
-    }
-}
-
 hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
@@ -323,7 +289,6 @@ hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 30: return launch_presto_rows<4, true, 8>(p, sh, st, io, stream);
             case 31: return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
             case 33: return launch_presto_rows<2, false, 8>(p, sh, st, io, stream);
-            case 40: return launch_presto_pipe<4>(p, sh, st, io, stream);
             case 50: return launch_presto_rows<2, true, -8>(p, sh, st, io, stream);
             case 35: return launch_presto_rows<2, true, 16>(p, sh, st, io, stream);
 
