@@ -63,11 +63,28 @@ hs_presto_generic_kernel(const __grid_constant__ HsShape sh, const __grid_consta
     float best = HS_NEG_INF;
     int bh = 0;
     for (int Hp = 1; Hp <= sh.H; Hp = all_o ? Hp + 1 : Hp * 2) {
-        const long long den = 2ll * Hp;
-        float sum = hs_load<HAS_BASE>(x, ib, (2ll * n + Hp) / den);          // fundamental
+        // Round(h n / H') = (2 h n + H') / (2 H') in exact integers (R3), advanced from h to h + step without a
+        // division per term: the numerator grows by 2 n step = (q_n 2 H' + r_n) step, q_n = n / H', r_n = 2 (n % H').
+        // (n < 2^31: 32-bit arithmetic; ONE division per H'.)
+        const unsigned den = 2u * Hp;
+        const unsigned qn = (unsigned)n / (unsigned)Hp, rn = 2u * ((unsigned)n - qn * Hp);
+        unsigned q = qn, r = rn + Hp;                                         // h = 1: (2 n + H') / (2 H')
+        if (r >= den) { r -= den; ++q; }
+        float sum = hs_load<HAS_BASE>(x, ib, q);                              // fundamental
         const int step = all_h ? 1 : 2;
-        for (int h = 2; h <= Hp; h += step)
-            sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, (2ll * h * n + Hp) / den));
+        // h = 2 is reached from h = 1 by one increment whatever the step
+        q += qn; r += rn;
+        if (r >= den) { r -= den; ++q; }
+        for (int h = 2; h <= Hp; h += step) {
+            sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, q));
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (k < step) {
+                    q += qn; r += rn;
+                    if (r >= den) { r -= den; ++q; }
+                }
+            }
+        }
         const float snr = hs_snr(sum, st.nmis[Hp - 1], st.inv_sigma[Hp - 1]);  // once per H' (R2)
         if (snr > best) { best = snr; bh = Hp; }
     }
