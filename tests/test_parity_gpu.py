@@ -317,6 +317,42 @@ def test_candidates_dense_and_batch(hs, oracle_mod):
         hs.hs_destroy(plan)
 
 
+def test_sensitivity_loss_workload(hs, oracle_mod):
+    """NEXT-3: the paper's noiseless sensitivity-loss experiment (eq. 10-11) as a second workload:
+    51 von Mises pulse trains stepping across one bin, 156 251 bins each (ragged), H = 32.  Parity against the oracle
+    for every variant, and the statements of the text as soft checks (figures 9-11 are not in PAPER.md)."""
+    from parity import check_greedy, check_presto
+    from paper_2202_12817_b200 import sensitivity as se
+    n_c, H = 500, 32
+    xt, _ = se.von_mises_spectra(n_c=n_c, device="cuda")
+    x = xt.cpu().numpy()
+    S, N = x.shape
+    assert (S, N) == (51, 156251)
+    # scalloping: a half-bin offset keeps |sinc(pi/2)|^2 = 0.405 of the bin-centred power (PAPER.md:76)
+    assert abs(x[25, n_c] / x[0, n_c] - (2.0 / np.pi) ** 2) < 0.01
+    mu = np.zeros(H, np.float32)
+    root = np.sqrt(np.arange(1, H + 1)).astype(np.float32)
+    pterms = np.sqrt([1.0 if h == 1 else 1.0 + h / 2.0 for h in range(1, H + 1)]).astype(np.float32)
+    loss, rsnr0 = {}, {}
+    for name, flags in (("greedy", 0), ("greedy_nofs", NO_FUND_SELECT), ("simple", NO_DRIFT)):
+        s, b, p = run_greedy(hs, x, H, mu, root, flags)
+        check_greedy(oracle_mod, x, H, mu, root, flags, s, b, p, T=None)
+        loss[name] = se.loss_curve(torch.from_numpy(s)).numpy()
+        rsnr0[name] = s[0, 10:].max()
+    for name, flags, sg in (("presto", 0, pterms), ("presto_all", ALL_HARMONICS, root), ("presto_plus", ALL_HARMONICS | ALL_ORDERS, root)):
+        s, b = run_presto(hs, x, H, mu, sg, flags)
+        check_presto(oracle_mod, x, H, mu, sg, flags, s, b, T=None)
+        loss[name] = se.loss_curve(torch.from_numpy(s)).numpy()
+        rsnr0[name] = s[0, 10:].max()
+    g, sm = loss["greedy"], loss["simple"]
+    assert abs(g[50] - 1.0) < 1e-3 and abs(sm[50] - 1.0) < 1e-3          # next bin centre: no loss
+    assert np.abs(g - g[::-1]).max() < 0.01                             # drift tracked: symmetric about the bin border (PAPER.md:290)
+    assert np.abs(loss["greedy_nofs"] - loss["greedy_nofs"][::-1]).max() > 0.1   # without fundamental selection it is not
+    assert g.min() > 0.65 and sm.min() < 0.5                            # simple HS loses about half (PAPER.md:366)
+    assert abs(rsnr0["greedy"] / rsnr0["presto_plus"] - 1.0) < 1e-4     # same maximum RSNR as PRESTO+ (PAPER.md:372)
+    assert rsnr0["presto"] < rsnr0["presto_all"] <= rsnr0["presto_plus"] * (1 + 1e-6)
+
+
 # ------------------------------------------------------------------------------------------
 # Host-buffer entry points (the e2e leg of bench.py) and error behaviour
 # ------------------------------------------------------------------------------------------
