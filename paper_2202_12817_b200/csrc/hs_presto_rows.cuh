@@ -142,6 +142,27 @@ __device__ __forceinline__ void stage_padded(float* __restrict__ sm, const float
     }
 }
 
+// The same for a span that ends inside the spectrum, with the per-thread address arithmetic done once:
+// float4 number q = t + j BLOCK lands at word (q / F4) P + 4 (q % F4), F4 = RL/4 float4s per row; BLOCK is a
+// multiple of F4, so q % F4 = t % F4 for every j and the destination advances by (BLOCK / F4) P words per j.
+template <int BLOCK, int KK, int W>
+__device__ __forceinline__ void stage_padded_interior(float* __restrict__ sm, const float* __restrict__ src_span) {
+    constexpr int RL = KK / 2, P = RL + 4, F4 = RL / 4, ROWS = 32 * W, Q = ROWS * F4, NJ = Q / BLOCK;
+    static_assert(Q % BLOCK == 0 && BLOCK % F4 == 0, "span shape");
+    const int t = threadIdx.x;
+    const unsigned dst = smem_u32(sm + (t / F4) * P + 4 * (t % F4));
+    const float* src = src_span + 4 * t;
+    const bool head = (t % F4) == 0;                                   // this float4 starts a row
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + 4u * (j * (BLOCK / F4) * P)), "l"(src + 4 * j * BLOCK) : "memory");
+        if (head && (j > 0 || t > 0))                                  // ... and is the tail of the row before
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + 4u * (j * (BLOCK / F4) * P) - 16u), "l"(src + 4 * j * BLOCK) : "memory");
+    }
+    if (t == 0)                                                        // the tail of the last row
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + 4u * (ROWS * P) - 16u), "l"(src + 4 * Q) : "memory");
+}
+
 // start of lane `lane` of warp `w`'s row in the span of fraction F
 template <int F, int W>
 __device__ __forceinline__ const float* row_ptr(const float* __restrict__ sm, int w, int lane) {
@@ -259,8 +280,8 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         }
     }
     if (interior) {
-        stage_padded<BLOCK, 32, W, true>(sm + span_off(0, W), x, 32 * b0, N);
-        if (L >= 1) stage_padded<BLOCK, 16, W, true>(sm + span_off(1, W), x, 16 * b0, N);
+        stage_padded_interior<BLOCK, 32, W>(sm + span_off(0, W), x + 32 * b0);
+        if (L >= 1) stage_padded_interior<BLOCK, 16, W>(sm + span_off(1, W), x + 16 * b0);
         asm volatile("cp.async.commit_group;\n cp.async.wait_group 0;\n" ::: "memory");
     } else {
         stage_padded<BLOCK, 32, W, false>(sm + span_off(0, W), x, 32 * b0, N);
@@ -305,6 +326,7 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     constexpr int V0 = 0, NV = PAIR ? 2 : 4;            // float4s of a row this warp writes / stream quarters it reads
     const int vbase = PAIR ? 2 * half : V0;
     auto sync_tile = [&]() { if (PAIR) __syncthreads(); else __syncwarp(); };
+    const bool full = n0 + T <= n_fund;                   // every output of the tile exists: no per-store checks
     sync_tile();
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
@@ -313,17 +335,25 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             make_float4(res_snr[4 * v], res_snr[4 * v + 1], res_snr[4 * v + 2], res_snr[4 * v + 3]);
     }
     sync_tile();
+    // float4 number q = lane + 32 (vbase + k) of the tile's output stream sits at row q / 4, words 4 (q % 4) ..
+    const float* rd = stg + ((lane >> 2) + 8 * vbase) * P + 4 * (lane & 3);
+    const long long o0 = orow + nw + 4 * (lane + 32 * vbase);
+    if (full) {
 #pragma unroll
-    for (int k = 0; k < NV; ++k) {
-        const int q = lane + 32 * (vbase + k);                        // float4 index in the tile's output stream
-        const float4 v = *reinterpret_cast<const float4*>(stg + (q >> 2) * P + 4 * (q & 3));
-        const int n = nw + 4 * q;
-        if (n + 3 < n_fund) {
-            __stcs(reinterpret_cast<float4*>(io.snr + orow + n), v);
-        } else {
-            if (n < n_fund) st_cs(io.snr + orow + n, v.x);
-            if (n + 1 < n_fund) st_cs(io.snr + orow + n + 1, v.y);
-            if (n + 2 < n_fund) st_cs(io.snr + orow + n + 2, v.z);
+        for (int k = 0; k < NV; ++k)
+            __stcs(reinterpret_cast<float4*>(io.snr + o0 + 128 * k), *reinterpret_cast<const float4*>(rd + 8 * k * P));
+    } else {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const float4 v = *reinterpret_cast<const float4*>(rd + 8 * k * P);
+            const int n = nw + 4 * (lane + 32 * (vbase + k));
+            if (n + 3 < n_fund) {
+                __stcs(reinterpret_cast<float4*>(io.snr + orow + n), v);
+            } else {
+                if (n < n_fund) st_cs(io.snr + orow + n, v.x);
+                if (n + 1 < n_fund) st_cs(io.snr + orow + n + 1, v.y);
+                if (n + 2 < n_fund) st_cs(io.snr + orow + n + 2, v.z);
+            }
         }
     }
     sync_tile();
@@ -334,17 +364,23 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             make_int4(res_bh[4 * v], res_bh[4 * v + 1], res_bh[4 * v + 2], res_bh[4 * v + 3]);
     }
     sync_tile();
+    const int* rdi = reinterpret_cast<const int*>(rd);
+    if (full) {
 #pragma unroll
-    for (int k = 0; k < NV; ++k) {
-        const int q = lane + 32 * (vbase + k);
-        const int4 v = *reinterpret_cast<const int4*>(stgi + (q >> 2) * P + 4 * (q & 3));
-        const int n = nw + 4 * q;
-        if (n + 3 < n_fund) {
-            __stcs(reinterpret_cast<int4*>(io.best_h + orow + n), v);
-        } else {
-            if (n < n_fund) st_cs(io.best_h + orow + n, v.x);
-            if (n + 1 < n_fund) st_cs(io.best_h + orow + n + 1, v.y);
-            if (n + 2 < n_fund) st_cs(io.best_h + orow + n + 2, v.z);
+        for (int k = 0; k < NV; ++k)
+            __stcs(reinterpret_cast<int4*>(io.best_h + o0 + 128 * k), *reinterpret_cast<const int4*>(rdi + 8 * k * P));
+    } else {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const int4 v = *reinterpret_cast<const int4*>(rdi + 8 * k * P);
+            const int n = nw + 4 * (lane + 32 * (vbase + k));
+            if (n + 3 < n_fund) {
+                __stcs(reinterpret_cast<int4*>(io.best_h + orow + n), v);
+            } else {
+                if (n < n_fund) st_cs(io.best_h + orow + n, v.x);
+                if (n + 1 < n_fund) st_cs(io.best_h + orow + n + 1, v.y);
+                if (n + 2 < n_fund) st_cs(io.best_h + orow + n + 2, v.z);
+            }
         }
     }
 }
