@@ -156,7 +156,20 @@ hs_status launch_greedy_band(hs_plan_s* p, const HsShape& full, const HsStats& s
 hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
-    const bool fast_ok = !(sh.flags & HS_GREEDY_NO_DRIFT) && sh.n_bins <= (1ll << 31) - 64 && p->tune != 255;
+    const bool no_drift = sh.flags & HS_GREEDY_NO_DRIFT;
+    const bool fast_ok = sh.n_bins <= (1ll << 31) - 64 && p->tune != 255 && (!no_drift || (!io.inv_base && p->tune <= 1));
+    if (fast_ok && no_drift) {                              // simple harmonic sum: the tile kernel without the second bin
+        const long long tile = 256 * 4;
+        dim3 grid((unsigned)((sh.n_fund + tile - 1) / tile), (unsigned)sh.n_spectra);
+        const bool fs = !(sh.flags & HS_GREEDY_NO_FUND_SELECT), wp = io.path != nullptr;
+        if (fs && wp) hs_greedy_tile_kernel<256, 4, true, true, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
+        else if (fs) hs_greedy_tile_kernel<256, 4, true, false, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
+        else if (wp) hs_greedy_tile_kernel<256, 4, false, true, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
+        else hs_greedy_tile_kernel<256, 4, false, false, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
+        p->launches += 1;
+        HS_CUDA(cudaGetLastError());
+        return HS_OK;
+    }
     if (fast_ok && !io.inv_base && p->d_mask && sh.n_bins <= (1ll << 30)) {
         switch (p->tune) {
             case 20: return launch_greedy_band<256, 1, 2>(p, sh, st, io, stream);

@@ -13,7 +13,8 @@
 #include "hs_common.cuh"
 
 // HAS_BASE: every x[b] is the fp32 product x[b] * inv_baseline[b] (reading R13; cfg4's whitening multiplier).
-template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false>
+// DRIFT = false: the simple harmonic sum (eq. 3; HS_GREEDY_NO_DRIFT): the second bin is never read.
+template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true>
 __global__ void __launch_bounds__(BLOCK)
 hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
     const int s = blockIdx.y;
@@ -45,7 +46,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             unsigned pb[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const bool shift = FUND_SELECT && e[k + 1] > e[k];  // strict >: ties stay
+                const bool shift = FUND_SELECT && DRIFT && e[k + 1] > e[k];  // strict >: ties stay
                 snr[k] = hs_snr(shift ? e[k + 1] : e[k], st.nmis[0], st.inv_sigma[0]);
                 pb[k] = shift ? 1u : 0u;
             }
@@ -81,10 +82,11 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             hn[j] += n[j];
             const int m = hn[j] + d[j];
             a[j] = __ldg(x + m);
-            b[j] = __ldg(x + m + 1);
-            if (HAS_BASE) {
-                a[j] = __fmul_rn(a[j], __ldg(ib + m));
-                b[j] = __fmul_rn(b[j], __ldg(ib + m + 1));
+            if (HAS_BASE) a[j] = __fmul_rn(a[j], __ldg(ib + m));
+            b[j] = HS_NEG_INF;
+            if (DRIFT) {
+                b[j] = __ldg(x + m + 1);
+                if (HAS_BASE) b[j] = __fmul_rn(b[j], __ldg(ib + m + 1));
             }
         }
 #pragma unroll
@@ -113,7 +115,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
                 float a = __ldg(x + m);
                 if (HAS_BASE) a = __fmul_rn(a, __ldg(ib + m));
                 float b = HS_NEG_INF;
-                if (m + 1 <= last && (FUND_SELECT || h != 1)) {
+                if (DRIFT && m + 1 <= last && (FUND_SELECT || h != 1)) {
                     b = __ldg(x + m + 1);
                     if (HAS_BASE) b = __fmul_rn(b, __ldg(ib + m + 1));
                 }

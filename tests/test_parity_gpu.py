@@ -120,13 +120,14 @@ def test_presto_exact_integer(hs, oracle_mod, tune, H):
         assert np.array_equal(s.astype(np.float64), s_ref), (S, N)
 
 
+@pytest.mark.parametrize("tune", [0, 1, 255])
 @pytest.mark.parametrize("flags", [NO_DRIFT, NO_DRIFT | NO_FUND_SELECT])
-def test_simple_hs_exact_integer(hs, oracle_mod, flags):
+def test_simple_hs_exact_integer(hs, oracle_mod, flags, tune):
     H = 16
     mu, sg = _int_stats(H)
     x = inputs.integer_spectra(7, 3, 5003, 255).numpy()
     s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags)
-    s, b, p = run_greedy(hs, x, H, mu, sg, flags)
+    s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16))
     assert np.all(p == 0) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
 
 
