@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-spectra", type=int, default=64, help="spectra in the oracle's bounded sample")
+    ap.add_argument("--H", type=int, default=0, help="override the workload's maximum harmonic order (paper Table 2: 4, 8, 16, 32)")
     ap.add_argument("--forms", default="both", choices=["both", "greedy", "presto"],
                     help="which forms a step runs (cfg4 is quoted on the greedy form only)")
     ap.add_argument("--greedy-flags", type=int, default=0, help="HS_GREEDY_* plan flags (NEXT-1 variants)")
@@ -215,7 +216,7 @@ def run_cuda(args):
     dev = torch.device("cuda", local)
     w = inputs.workload(args.workload)
     S = args.spectra or w.n_spectra
-    N, H = w.n_bins, w.H
+    N, H = w.n_bins, (args.H or w.H)
     # rank r owns global rows [r*S, (r+1)*S): weak scaling, no exchange
     x = torch.empty((S, N), dtype=torch.float32, device=dev)
     for s in range(S):
