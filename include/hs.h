@@ -39,7 +39,9 @@
  *        snr = (sum - mu[H'-1]) / sigma[H'-1];  if snr > best { best = snr; best_h = H' }
  *   With d_inv_baseline != NULL every x[b] above is replaced by the fp32 product
  *   x[b] * inv_baseline[b] (spectrum whitening supplied by the caller).
- *   Sums are accumulated in fp32 in the order written above; the SNR is formed as
+ *   Sums are accumulated in fp32 in the order written above (for the ALL_HARMONICS variants the terms of
+ *   one H' may instead be grouped by reduced fraction h/H', each group in increasing h, groups in
+ *   increasing denominator); the SNR is formed as
  *   fma(sum, 1/sigma, -mu/sigma) in fp32, both constants rounded once on the host.  Non-finite
  *   inputs give unspecified results.
  *

@@ -15,6 +15,7 @@
 #include "hs_presto.cuh"
 #include "hs_presto_smem.cuh"
 #include "hs_presto_rows.cuh"
+#include "hs_presto_farey.cuh"
 #include "hs_candidates.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
@@ -281,6 +282,16 @@ hs_status launch_presto_rows(hs_plan_s* p, const HsShape& sh, const HsStats& st,
 hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
+    // PRESTO_all, and PRESTO+ at H > 16 (measured: below that the coverage kernel is faster): hs_presto_farey.cuh
+    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && p->tune != 255 &&
+        (!(sh.flags & HS_PRESTO_ALL_ORDERS) || sh.H > 16 || p->tune == 1)) {
+        dim3 fgrid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
+        if (sh.flags & HS_PRESTO_ALL_ORDERS) hs_presto_farey_kernel<true><<<fgrid, 256, 0, stream>>>(sh, st, io);
+        else hs_presto_farey_kernel<false><<<fgrid, 256, 0, stream>>>(sh, st, io);
+        p->launches += 1;
+        HS_CUDA(cudaGetLastError());
+        return HS_OK;
+    }
     const bool fast_ok = !io.inv_base && !(sh.flags & (HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS)) &&
                          sh.n_bins * 32 < (1ll << 31) - 64 && p->tune != 255;
     if (fast_ok) {

@@ -131,14 +131,16 @@ def test_simple_hs_exact_integer(hs, oracle_mod, flags, tune):
     assert np.all(p == 0) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
 
 
+@pytest.mark.parametrize("tune", [0, 1, 255])       # library choice / Farey kernel forced / generic kernel
 @pytest.mark.parametrize("flags", [ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS])
-@pytest.mark.parametrize("H", [5, 16, 32])
-def test_presto_variants_exact_integer(hs, oracle_mod, flags, H):
+@pytest.mark.parametrize("H", [1, 2, 5, 16, 27, 32])
+def test_presto_variants_exact_integer(hs, oracle_mod, flags, H, tune):
     mu, sg = _int_stats(H)
-    x = inputs.integer_spectra(8, 2, 6007, 255).numpy()
-    s_ref, b_ref = oracle_mod.presto(x, H, mu, sg, flags)
-    s, b = run_presto(hs, x, H, mu, sg, flags)
-    assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
+    for S, N in ((2, 6007), (1, 2), (3, 257), (2, 70001)):
+        x = inputs.integer_spectra(8 + N, S, N, 255).numpy()
+        s_ref, b_ref = oracle_mod.presto(x, H, mu, sg, flags)
+        s, b = run_presto(hs, x, H, mu, sg, flags | (tune << 16))
+        assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref), (S, N)
 
 
 def test_strides_and_n_fund(hs, oracle_mod):
