@@ -19,8 +19,9 @@
 //   * 15 spans are copied as they are by one 1-D bulk async copy each (TMA engine, cp.async.bulk ->
 //     UBLKCP): the lane stride kk/2 words makes their vector loads bank-conflict free;
 //   * for kk = 32 and kk = 16 a lane stride of 16 / 8 words would serialise the 16-byte loads 4- / 2-fold,
-//     so those two spans are stored as padded rows (pitch 20 / 12 words, the 4 words of padding repeat
-//     the head of the next row) by a coalesced LDG.128 -> STS.128 pass of the whole CTA.
+//     so those two spans are stored as padded rows by coalesced 16-byte cp.async copies of the whole CTA:
+//     kk = 16 with a pitch of 12 words (the 4 words of padding repeat the head of the next row), kk = 32 as
+//     pairs of 16-word rows sharing one 16-byte pad (row32_off: conflict-free lane-major AND stream-major).
 // The outputs of a lane are consecutive too; they go back through the warp's own kk = 32 rows
 // (dead by then) so that the global stores are coalesced 16-byte streaming stores.
 #pragma once
@@ -40,9 +41,14 @@ __host__ __device__ constexpr int frac_kk(int f) {
 __host__ __device__ constexpr int frac_level(int f) { return f == 0 ? 0 : f == 1 ? 1 : f == 2 ? 2 : f <= 4 ? 3 : f <= 8 ? 4 : 5; }
 __host__ __device__ constexpr bool frac_padded(int kk) { return kk == 32 || kk == 16; }
 __host__ __device__ constexpr int pad_pitch(int kk) { return kk / 2 + 4; }
+// kk = 32 (x[n] itself; its rows are also the transposition buffer of the output pass): row r holds exactly the 16
+// words of lane r, two rows share 9 sixteen-byte units (8 of data + 1 of padding).  Both ways the rows are touched
+// are then bank-conflict free: lane-major (lane i reads / writes unit c of row i: 9 (i >> 1) + 4 (i & 1) + c are
+// distinct mod 8 over 8 lanes) and stream-major (consecutive lanes take consecutive units of the row pairs).
+__host__ __device__ constexpr int row32_off(int r) { return 36 * (r >> 1) + 16 * (r & 1); }
 // words of shared memory of one span of a CTA tile of W warps
 __host__ __device__ constexpr int span_words(int kk, int W) {
-    return frac_padded(kk) ? 32 * W * pad_pitch(kk) : 16 * kk * W + 4;
+    return kk == 32 ? 18 * 32 * W : frac_padded(kk) ? 32 * W * pad_pitch(kk) : 16 * kk * W + 4;
 }
 __host__ __device__ constexpr int span_off(int f, int W) {
     int o = 0;
@@ -163,10 +169,38 @@ __device__ __forceinline__ void stage_padded_interior(float* __restrict__ sm, co
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + 4u * (ROWS * P) - 16u), "l"(src + 4 * Q) : "memory");
 }
 
+// kk = 32 rows (row32_off layout) of a tile of W warps: float4 number q of the span x[g ..] is unit q & 3 of row q >> 2
+template <int BLOCK, int W, bool INTERIOR>
+__device__ __forceinline__ void stage_x32(float* __restrict__ sm, const float* __restrict__ x, int g, int N) {
+    constexpr int Q = 32 * W * 4, NJ = Q / BLOCK;
+    static_assert(Q % BLOCK == 0 && BLOCK % 8 == 0, "span shape");
+    const int t = threadIdx.x;
+    float* d0 = sm + row32_off(t >> 2) + 4 * (t & 3);             // + 36 BLOCK / 8 words per j
+    if (INTERIOR) {
+        const unsigned dst = smem_u32(d0);
+        const float* src = x + g + 4 * t;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + 4u * (j * (36 * BLOCK / 8))), "l"(src + 4 * j * BLOCK) : "memory");
+    } else {
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int e = g + 4 * (t + j * BLOCK);
+            float4 v;
+            v.x = (e < N) ? __ldg(x + e) : 0.f;
+            v.y = (e + 1 < N) ? __ldg(x + e + 1) : 0.f;
+            v.z = (e + 2 < N) ? __ldg(x + e + 2) : 0.f;
+            v.w = (e + 3 < N) ? __ldg(x + e + 3) : 0.f;
+            *reinterpret_cast<float4*>(d0 + j * (36 * BLOCK / 8)) = v;
+        }
+    }
+}
+
 // start of lane `lane` of warp `w`'s row in the span of fraction F
 template <int F, int W>
 __device__ __forceinline__ const float* row_ptr(const float* __restrict__ sm, int w, int lane) {
     constexpr int kk = frac_kk(F);
+    if (kk == 32) return sm + span_off(F, W) + row32_off(32 * w + lane);
     if (frac_padded(kk)) return sm + span_off(F, W) + (32 * w + lane) * pad_pitch(kk);
     if (kk == 1) return sm + span_off(F, W) + 16 * w + ((lane + 1) >> 1);
     return sm + span_off(F, W) + 16 * kk * w + (kk / 2) * lane;
@@ -280,11 +314,11 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         }
     }
     if (interior) {
-        stage_padded_interior<BLOCK, 32, W>(sm + span_off(0, W), x + 32 * b0);
+        stage_x32<BLOCK, W, true>(sm + span_off(0, W), x, 32 * b0, N);
         if (L >= 1) stage_padded_interior<BLOCK, 16, W>(sm + span_off(1, W), x + 16 * b0);
         asm volatile("cp.async.commit_group;\n cp.async.wait_group 0;\n" ::: "memory");
     } else {
-        stage_padded<BLOCK, 32, W, false>(sm + span_off(0, W), x, 32 * b0, N);
+        stage_x32<BLOCK, W, false>(sm + span_off(0, W), x, 32 * b0, N);
         if (L >= 1) stage_padded<BLOCK, 16, W, false>(sm + span_off(1, W), x, 16 * b0, N);
     }
     __syncthreads();
@@ -318,8 +352,7 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     }
 
     // ---- store: transpose through the tile's own kk = 32 rows (32 rows x pitch 20, no longer read) ----
-    constexpr int P = pad_pitch(32);
-    float* stg = sm + span_off(0, W) + 32 * w * P;
+    float* stg = sm + span_off(0, W) + row32_off(32 * w);
     int* stgi = reinterpret_cast<int*>(stg);
     const long long orow = (long long)s * sh.out_stride;
     const int nw = n0 + WT * w;
@@ -331,21 +364,21 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
         const int col = PAIR ? 8 * half + 4 * v : 4 * v;
-        *reinterpret_cast<float4*>(stg + lane * P + col) =
+        *reinterpret_cast<float4*>(stg + row32_off(lane) + col) =
             make_float4(res_snr[4 * v], res_snr[4 * v + 1], res_snr[4 * v + 2], res_snr[4 * v + 3]);
     }
     sync_tile();
     // float4 number q = lane + 32 (vbase + k) of the tile's output stream sits at row q / 4, words 4 (q % 4) ..
-    const float* rd = stg + ((lane >> 2) + 8 * vbase) * P + 4 * (lane & 3);
+    const float* rd = stg + row32_off((lane >> 2) + 8 * vbase) + 4 * (lane & 3);   // + 8 rows = 144 words per k
     const long long o0 = orow + nw + 4 * (lane + 32 * vbase);
     if (full) {
 #pragma unroll
         for (int k = 0; k < NV; ++k)
-            __stcs(reinterpret_cast<float4*>(io.snr + o0 + 128 * k), *reinterpret_cast<const float4*>(rd + 8 * k * P));
+            __stcs(reinterpret_cast<float4*>(io.snr + o0 + 128 * k), *reinterpret_cast<const float4*>(rd + 144 * k));
     } else {
 #pragma unroll
         for (int k = 0; k < NV; ++k) {
-            const float4 v = *reinterpret_cast<const float4*>(rd + 8 * k * P);
+            const float4 v = *reinterpret_cast<const float4*>(rd + 144 * k);
             const int n = nw + 4 * (lane + 32 * (vbase + k));
             if (n + 3 < n_fund) {
                 __stcs(reinterpret_cast<float4*>(io.snr + orow + n), v);
@@ -360,7 +393,7 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
         const int col = PAIR ? 8 * half + 4 * v : 4 * v;
-        *reinterpret_cast<int4*>(stgi + lane * P + col) =
+        *reinterpret_cast<int4*>(stgi + row32_off(lane) + col) =
             make_int4(res_bh[4 * v], res_bh[4 * v + 1], res_bh[4 * v + 2], res_bh[4 * v + 3]);
     }
     sync_tile();
@@ -368,11 +401,11 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     if (full) {
 #pragma unroll
         for (int k = 0; k < NV; ++k)
-            __stcs(reinterpret_cast<int4*>(io.best_h + o0 + 128 * k), *reinterpret_cast<const int4*>(rdi + 8 * k * P));
+            __stcs(reinterpret_cast<int4*>(io.best_h + o0 + 128 * k), *reinterpret_cast<const int4*>(rdi + 144 * k));
     } else {
 #pragma unroll
         for (int k = 0; k < NV; ++k) {
-            const int4 v = *reinterpret_cast<const int4*>(rdi + 8 * k * P);
+            const int4 v = *reinterpret_cast<const int4*>(rdi + 144 * k);
             const int n = nw + 4 * (lane + 32 * (vbase + k));
             if (n + 3 < n_fund) {
                 __stcs(reinterpret_cast<int4*>(io.best_h + orow + n), v);
