@@ -283,7 +283,8 @@ hs_presto_rows_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int n_fund = (int)sh.n_fund;
     const int n0 = blockIdx.x * T;
     const int b0 = blockIdx.x * (T / 32);               // n0 / 32: span of fraction kk starts at element kk b0
-    const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
+    const float* x = io.x + (long long)s * sh.in_stride;
+    asm volatile("" : "+l"(x));                                  // one materialised row pointer for all the copies
 
     // ---- stage ----
     const bool interior = BULK && (n0 + T + 4 <= N);    // every span (the longest is kk = 32) ends inside the row
