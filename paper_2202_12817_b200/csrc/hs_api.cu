@@ -316,7 +316,9 @@ hs_status launch_presto(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 50: return launch_presto_rows<2, true, -8>(p, sh, st, io, stream);
             case 35: return launch_presto_rows<2, true, 16>(p, sh, st, io, stream);
 
-            default: return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
+            default:                                        // measured: two warps per tile win at H >= 32 only
+                if (sh.H >= 32) return launch_presto_rows<2, true, -8>(p, sh, st, io, stream);
+                return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
