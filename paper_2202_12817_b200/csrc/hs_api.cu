@@ -158,7 +158,8 @@ hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
     if (sh.n_fund == 0) return HS_OK;
     if (sh.n_spectra > 65535) return HS_ERR_UNSUPPORTED;
     const bool no_drift = sh.flags & HS_GREEDY_NO_DRIFT;
-    const bool fast_ok = sh.n_bins <= (1ll << 31) - 64 && p->tune != 255 && (!no_drift || (!io.inv_base && p->tune <= 1));
+    // the tile kernel keeps h n in 32 bits: h n < N + 32 * (tile of 1024 fundamentals)
+    const bool fast_ok = sh.n_bins <= (1ll << 31) - (1ll << 17) && p->tune != 255 && (!no_drift || (!io.inv_base && p->tune <= 1));
     if (fast_ok && no_drift) {                              // simple harmonic sum: the tile kernel without the second bin
         const long long tile = 256 * 4;
         dim3 grid((unsigned)((sh.n_fund + tile - 1) / tile), (unsigned)sh.n_spectra);

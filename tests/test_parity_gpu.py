@@ -452,3 +452,51 @@ def test_cfg3_full_size_sampled_rows(hs, oracle_mod):
         check_presto(oracle_mod, xs, H, mu, sg, 0, snr[rows].cpu().numpy(), bh[rows].cpu().numpy(), T=10.0)
     finally:
         hs.hs_destroy(plan)
+
+
+def _sample_bins(N, rng, k=6000):
+    edges = np.concatenate([np.arange(0, 64), np.arange(N - 64, N)] +
+                           [np.arange(max(0, N // d - 40), min(N, N // d + 40)) for d in (2, 3, 4, 8, 16, 31, 32, 33, 64)])
+    return np.unique(np.concatenate([edges, rng.integers(0, N, size=k), rng.integers(0, max(1, N // 32), size=k)]))
+
+
+def test_maximum_sizes_sampled(hs, oracle_mod):
+    """Largest rows the fast paths accept: greedy tile kernel at N = 2^30 + 7 (32-bit h n close to its limit), PRESTO
+    rows kernel at N = 2^26 - 70 (32 N just below 2^31).  Exact-integer spectra, so sampled outputs must equal the
+    oracle's bit for bit (the oracle computes the sampled bins one by one)."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 30 * (1 << 30):
+        pytest.skip("needs 30 GiB of device memory")
+    H = 32
+    mu, sg = _int_stats(H)
+    rng = np.random.default_rng(11)
+    for kind, N in (("greedy", (1 << 30) + 7), ("presto", (1 << 26) - 70)):
+        g = torch.Generator(device="cuda"); g.manual_seed(5)
+        istr = (N + 3) & ~3
+        x = torch.zeros((1, istr), dtype=torch.float32, device="cuda")
+        x[0, :N] = torch.randint(0, 256, (N,), generator=g, device="cuda", dtype=torch.int32).to(torch.float32)
+        snr = torch.empty((1, istr), dtype=torch.float32, device="cuda")
+        bh = torch.empty((1, istr), dtype=torch.int32, device="cuda")
+        path = torch.empty((1, istr), dtype=torch.int32, device="cuda") if kind == "greedy" else None
+        plan = hs.hs_plan(N, 1, H, istr, istr, 0, 0, 0)
+        try:
+            if kind == "greedy":
+                hs.hs_run_greedy(plan, x, None, mu, sg, snr, bh, path)
+            else:
+                hs.hs_run_presto(plan, x, None, mu, sg, snr, bh)
+            torch.cuda.synchronize()
+        finally:
+            hs.hs_destroy(plan)
+        bins = _sample_bins(N, rng)
+        idx = torch.from_numpy(bins).cuda()
+        xh = x[0, :N].cpu().numpy()[None, :]
+        rows = np.zeros_like(bins)
+        if kind == "greedy":
+            ref = oracle_mod.greedy_bins(xh, H, mu, sg, rows, bins)
+            assert np.array_equal(path[0, idx].cpu().numpy().view(np.uint32), ref["path"])
+        else:
+            ref = oracle_mod.presto_bins(xh, H, mu, sg, rows, bins)
+        assert np.array_equal(bh[0, idx].cpu().numpy(), ref["best_h"])
+        assert np.array_equal(snr[0, idx].cpu().numpy().astype(np.float64), ref["snr"])
+        del x, snr, bh, path, xh
+        torch.cuda.empty_cache()
