@@ -161,13 +161,13 @@ hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
     // the tile kernel keeps h n in 32 bits: h n < N + 32 * (tile of 1024 fundamentals)
     const bool fast_ok = sh.n_bins <= (1ll << 31) - (1ll << 17) && p->tune != 255 && (!no_drift || (!io.inv_base && p->tune <= 1));
     if (fast_ok && no_drift) {                              // simple harmonic sum: the tile kernel without the second bin
-        const long long tile = 256 * 4;
+        const long long tile = 128 * 4;
         dim3 grid((unsigned)((sh.n_fund + tile - 1) / tile), (unsigned)sh.n_spectra);
         const bool fs = !(sh.flags & HS_GREEDY_NO_FUND_SELECT), wp = io.path != nullptr;
-        if (fs && wp) hs_greedy_tile_kernel<256, 4, true, true, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
-        else if (fs) hs_greedy_tile_kernel<256, 4, true, false, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
-        else if (wp) hs_greedy_tile_kernel<256, 4, false, true, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
-        else hs_greedy_tile_kernel<256, 4, false, false, false, false><<<grid, 256, 0, stream>>>(sh, st, io);
+        if (fs && wp) hs_greedy_tile_kernel<128, 4, true, true, false, false><<<grid, 128, 0, stream>>>(sh, st, io);
+        else if (fs) hs_greedy_tile_kernel<128, 4, true, false, false, false><<<grid, 128, 0, stream>>>(sh, st, io);
+        else if (wp) hs_greedy_tile_kernel<128, 4, false, true, false, false><<<grid, 128, 0, stream>>>(sh, st, io);
+        else hs_greedy_tile_kernel<128, 4, false, false, false, false><<<grid, 128, 0, stream>>>(sh, st, io);
         p->launches += 1;
         HS_CUDA(cudaGetLastError());
         return HS_OK;
@@ -197,7 +197,7 @@ hs_status launch_greedy(hs_plan_s* p, const HsShape& sh, const HsStats& st, cons
             case 6: return launch_greedy_tile<128, 4>(p, sh, st, io, stream);
             case 7: return launch_greedy_tile<512, 1>(p, sh, st, io, stream);
             case 8: return launch_greedy_tile<512, 2>(p, sh, st, io, stream);
-            default: return launch_greedy_tile<256, 4>(p, sh, st, io, stream);
+            default: return launch_greedy_tile<128, 4>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);

@@ -15,7 +15,7 @@
 // HAS_BASE: every x[b] is the fp32 product x[b] * inv_baseline[b] (reading R13; cfg4's whitening multiplier).
 // DRIFT = false: the simple harmonic sum (eq. 3; HS_GREEDY_NO_DRIFT): the second bin is never read.
 template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true>
-__global__ void __launch_bounds__(BLOCK, (BLOCK == 256 && R == 4) ? 6 : 1)
+__global__ void __launch_bounds__(BLOCK, (R == 4) ? 1536 / BLOCK : 1)
 hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
     const int s = blockIdx.y;
     const int N = (int)sh.n_bins;
