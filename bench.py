@@ -35,7 +35,7 @@ BYTES_PER_BIN = 12.0          # compulsory HBM bytes per bin and per form: 4 rea
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), keyed by kernel family; None until a capture exists.
-NCU_TRAFFIC_BYTES = {"greedy": 4.297286e9 + 8.539277e9, "presto": 4.296142e9 + 8.535727e9}   # profiles/r01b_ncu_full_summary.md, captures D / E
+NCU_TRAFFIC_BYTES = {"greedy": 4.295696e9 + 8.540868e9, "presto": 4.296142e9 + 8.535727e9}   # profiles/r01b_ncu_full_summary.md, captures E / F
 
 
 def parse_args():
