@@ -191,6 +191,54 @@ def test_p5_presto_bruteforce_exact_rational(oracle_mod, flags):
                 assert s[0, n] == float(best) and b[0, n] == bh, (seed, H, n)
 
 
+def _path_tree(y, n, H, flags):
+    """All monotone drift paths of fundamental n through the values y (Fig. 4).
+    Returns (locally greedy paths [(bits, partial sums)], best partial sum over all paths per order)."""
+    N = len(y)
+    greedy_paths, best_sum_at = [], [-math.inf] * H
+    for bits in range(1 << H):
+        d, tot, in_tree, locally_greedy, sums = 0, 0.0, True, True, []
+        for h in range(1, H + 1):
+            m = h * n + d
+            step = (bits >> (h - 1)) & 1
+            if m > N - 1:                       # band edge: the path ends here (R4)
+                in_tree = in_tree and (bits >> (h - 1)) == 0   # canonical: no later steps
+                break
+            second = float(y[m + 1]) if m + 1 <= N - 1 else None
+            if h == 1 and (flags & NO_FUND_SELECT):
+                second = None                   # the tree has a single child here (R7)
+            if step and second is None:
+                in_tree = False
+                break
+            want = 1 if (second is not None and second > float(y[m])) else 0
+            locally_greedy = locally_greedy and (step == want)
+            tot += second if step else float(y[m])
+            d += step
+            sums.append(tot)
+        if not in_tree:
+            continue
+        for i, t in enumerate(sums):
+            best_sum_at[i] = max(best_sum_at[i], t)
+        if locally_greedy:
+            greedy_paths.append((bits, sums))
+    return greedy_paths, best_sum_at
+
+
+def _check_against_tree(res, y, N, H, flags, mu, sg, tag):
+    for n in range(N):
+        greedy_paths, best_sum_at = _path_tree(y, n, H, flags)
+        assert len(greedy_paths) == 1, (tag, n)
+        bits, sums = greedy_paths[0]
+        assert res["path"][n] == bits, (tag, n)
+        got = res["snr_h"][n] * sg + mu           # partial sums back from the per-order SNRs
+        for i, t in enumerate(sums):
+            assert got[i] == t and t <= best_sum_at[i]
+        assert np.all(np.isnan(res["snr_h"][n][len(sums):]))
+        snrs = [(t - mu[i]) / sg[i] for i, t in enumerate(sums)]
+        assert res["snr"][n] == max(snrs)
+        assert res["best_h"][n] == 1 + snrs.index(max(snrs))      # first maximum (R6)
+
+
 @pytest.mark.parametrize("flags", [0, NO_FUND_SELECT])
 def test_p5_greedy_bruteforce_path_tree(oracle_mod, flags):
     """Enumerate all 2^H monotone drift paths of the tree (Fig. 4).  Exactly one
@@ -201,43 +249,81 @@ def test_p5_greedy_bruteforce_path_tree(oracle_mod, flags):
         mu = np.arange(1, H + 1).astype(np.float32)
         sg = np.ones(H, np.float32)
         res = oracle_mod.greedy_bins(x, H, mu, sg, [0] * N, list(range(N)), flags)
-        for n in range(N):
-            greedy_paths, best_sum_at = [], [-math.inf] * H
-            for bits in range(1 << H):
-                d, tot, in_tree, locally_greedy, sums = 0, 0.0, True, True, []
-                for h in range(1, H + 1):
-                    m = h * n + d
-                    step = (bits >> (h - 1)) & 1
-                    if m > N - 1:                       # band edge: the path ends here (R4)
-                        in_tree = in_tree and (bits >> (h - 1)) == 0   # canonical: no later steps
-                        break
-                    second = float(x[m + 1]) if m + 1 <= N - 1 else None
-                    if h == 1 and (flags & NO_FUND_SELECT):
-                        second = None                   # the tree has a single child here (R7)
-                    if step and second is None:
-                        in_tree = False
-                        break
-                    want = 1 if (second is not None and second > float(x[m])) else 0
-                    locally_greedy = locally_greedy and (step == want)
-                    tot += second if step else float(x[m])
-                    d += step
-                    sums.append(tot)
-                if not in_tree:
-                    continue
-                for i, t in enumerate(sums):
-                    best_sum_at[i] = max(best_sum_at[i], t)
-                if locally_greedy:
-                    greedy_paths.append((bits, sums))
-            assert len(greedy_paths) == 1, (seed, n)
-            bits, sums = greedy_paths[0]
-            assert res["path"][n] == bits
-            got = res["snr_h"][n] * sg + mu           # partial sums back from the per-order SNRs
-            for i, t in enumerate(sums):
-                assert got[i] == t and t <= best_sum_at[i]
-            assert np.all(np.isnan(res["snr_h"][n][len(sums):]))
-            snrs = [(t - mu[i]) / sg[i] for i, t in enumerate(sums)]
-            assert res["snr"][n] == max(snrs)
-            assert res["best_h"][n] == 1 + snrs.index(max(snrs))      # first maximum (R6)
+        _check_against_tree(res, x, N, H, flags, mu, sg, seed)
+
+
+# ------------------------------------------------------------------------------------------
+# R13 / NEXT-2  the whitening multiplier: every x[b] is replaced by the fp32 product x[b] * inv_baseline[b]
+# ("whitening" happens before the sum; PAPER.md:264 same pre-processing for all algorithms)
+# ------------------------------------------------------------------------------------------
+def test_r13_inv_baseline_power_of_two_equals_premultiplied(oracle_mod):
+    """With power-of-two multipliers the product is exact in fp32, so running on (x, ib) must equal
+    running on the pre-multiplied spectrum bit for bit -- and differ from ignoring ib."""
+    rng = np.random.default_rng(41)
+    S, N, H = 3, 1500, 8
+    x = rng.exponential(1.0, (S, N)).astype(np.float32)
+    ib = (2.0 ** rng.integers(-3, 4, (S, N))).astype(np.float32)
+    y = x * ib                                                # exact
+    assert np.array_equal(y.astype(np.float64), x.astype(np.float64) * ib.astype(np.float64))
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+    bins = np.arange(0, N, 3)
+    rows = bins % S
+    for flags in (0, NO_FUND_SELECT, NO_DRIFT):
+        a = oracle_mod.greedy(x, H, mu, sg, flags, inv_baseline=ib)
+        b = oracle_mod.greedy(y, H, mu, sg, flags)
+        c = oracle_mod.greedy(x, H, mu, sg, flags)
+        for u, v in zip(a, b):
+            assert np.array_equal(u, v)
+        assert not np.array_equal(a[0], c[0])                 # the multiplier is not ignored
+        ra = oracle_mod.greedy_bins(x, H, mu, sg, rows, bins, flags, inv_baseline=ib)
+        rb = oracle_mod.greedy_bins(y, H, mu, sg, rows, bins, flags)
+        for k in ("snr", "best_h", "path", "bin_h"):
+            assert np.array_equal(ra[k], rb[k]), k
+        assert np.array_equal(ra["snr_h"], rb["snr_h"], equal_nan=True)
+        assert np.array_equal(ra["snr"], a[0][rows, bins])
+    for flags in (0, ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS):
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("presto" if flags == 0 else "presto_plus", H))
+        a = oracle_mod.presto(x, H, mu, sg, flags, inv_baseline=ib)
+        b = oracle_mod.presto(y, H, mu, sg, flags)
+        c = oracle_mod.presto(x, H, mu, sg, flags)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+        assert not np.array_equal(a[0], c[0])
+        ra = oracle_mod.presto_bins(x, H, mu, sg, rows, bins, flags, inv_baseline=ib)
+        rb = oracle_mod.presto_bins(y, H, mu, sg, rows, bins, flags)
+        assert np.array_equal(ra["snr"], rb["snr"]) and np.array_equal(ra["best_h"], rb["best_h"])
+        assert np.array_equal(ra["snr_h"], rb["snr_h"], equal_nan=True)
+
+
+@pytest.mark.parametrize("flags", [0, NO_FUND_SELECT])
+def test_r13_inv_baseline_flips_comparisons_path_tree(oracle_mod, flags):
+    """Small-integer x and ib (products exact): the multiplier must change WHICH child is larger; the
+    oracle's path is the unique locally greedy path of the tree over the products, which differs from
+    the tree over x alone."""
+    for seed, N, H in ((8, 40, 5), (9, 57, 6)):
+        rng = np.random.default_rng(seed)
+        x = rng.integers(1, 6, N).astype(np.float32)
+        ib = rng.integers(1, 5, N).astype(np.float32)
+        y = [float(a) * float(b) for a, b in zip(x, ib)]       # exact small integers
+        mu = np.arange(1, H + 1).astype(np.float32)
+        sg = np.ones(H, np.float32)
+        res = oracle_mod.greedy_bins(x, H, mu, sg, [0] * N, list(range(N)), flags, inv_baseline=ib)
+        _check_against_tree(res, y, N, H, flags, mu, sg, seed)
+        plain = oracle_mod.greedy_bins(x, H, mu, sg, [0] * N, list(range(N)), flags)
+        assert np.count_nonzero(plain["path"] != res["path"]) >= 8          # comparisons really flipped
+
+
+def test_r13_inv_baseline_product_is_one_fp32_multiply(oracle_mod):
+    """The product that decides the comparison is rounded to fp32 (reading R13): two fp64-distinct
+    products that round to the same fp32 value tie, and a tie stays."""
+    a, ia = np.float32(1.0 + 2.0 ** -23), np.float32(3.0)    # exact product 3 + 1.5 ulp: rounds (to even) to 3 + 2 ulp
+    b, ib_ = np.float32(3.0 + 2.0 ** -21), np.float32(1.0)   # 3 + 2 ulp
+    pa64, pb64 = float(a) * float(ia), float(b) * float(ib_)
+    assert pb64 > pa64 and np.float32(a * ia) == np.float32(b * ib_)       # fp64: second larger; fp32: tie
+    x = np.array([a, b, 0.0, 0.0], np.float32)
+    ib = np.array([ia, ib_, 1.0, 1.0], np.float32)
+    r = oracle_mod.greedy_bins(x, 1, [0.0], [1.0], [0], [0], inv_baseline=ib)
+    assert r["path"][0] == 0 and r["bin_h"][0, 0] == 0
+    assert r["snr"][0] == float(np.float32(a * ia))
 
 
 # ------------------------------------------------------------------------------------------
