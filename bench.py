@@ -33,9 +33,20 @@ METRIC = "harmonic-sum spectrum bins/s at H=32 (greedy + PRESTO-like forms per b
 UNIT = "bins/s"
 BYTES_PER_BIN = 12.0          # compulsory HBM bytes per bin and per form: 4 read + 4 + 4 written
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/), keyed by kernel family; None until a capture exists.
-NCU_TRAFFIC_BYTES = {"greedy": 4.295696e9 + 8.540868e9, "presto": 4.296142e9 + 8.535727e9}   # profiles/r01b_ncu_full_summary.md, captures E / F
+# Committed ncu evidence: profiles/ncu_kernels.json maps the name hs_last_kernel() reports to the per-launch
+# counters of the `ncu --set full` capture of that kernel on cfg3 (dram bytes, L2 -> SM sectors);
+# profiles/machine_model.json holds the measured L2 -> SM ceiling.  A kernel that is not in the file gets
+# traffic = null (no stale numbers).
+NCU_KERNELS_JSON = os.path.join(ROOT, "profiles", "ncu_kernels.json")
+MACHINE_MODEL_JSON = os.path.join(ROOT, "profiles", "machine_model.json")
+
+
+def _load_json(path):
+    try:
+        with open(path) as f:
+            return json.load(f)
+    except Exception:
+        return {}
 
 
 def parse_args():
@@ -121,10 +132,26 @@ class ClockSampler:
         return out
 
 
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` (N > 1) outside torchrun: start the N ranks ourselves, one per GPU."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
 def dist_setup(n_gpus: int):
     import torch
     import torch.distributed as dist
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != max(1, n_gpus):
+        raise SystemExit(f"bench.py: --gpus {n_gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node {n_gpus} "
+                         f"(or run `python bench.py --gpus {n_gpus}` outside torchrun: it starts the ranks itself)")
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if world > 1:
@@ -235,8 +262,10 @@ def run_cuda(args):
     gv, fs, pv = _variants(args)
     mu_g, sg_g = inputs.exp1_stats(gv, H, fs)
     mu_p, sg_p = inputs.exp1_stats(pv, H)
-    plan_g = hs.hs_plan(N, S, H, flags=args.greedy_flags | (args.tune_greedy << hs.HS_TUNE_SHIFT), device=local)
-    plan_p = hs.hs_plan(N, S, H, flags=args.presto_flags | (args.tune_presto << hs.HS_TUNE_SHIFT), device=local)
+    plan_g = hs.hs_plan(N, S, H, flags=args.greedy_flags, device=local)
+    plan_p = hs.hs_plan(N, S, H, flags=args.presto_flags, device=local)
+    hs.hs_plan_set_tuning(plan_g, args.tune_greedy)     # 0 = the library's choice (diagnostic knob)
+    hs.hs_plan_set_tuning(plan_p, args.tune_presto)
     stream = torch.cuda.current_stream(dev)
 
     def step(ev=None):
@@ -264,6 +293,7 @@ def run_cuda(args):
         step(evs[k])
     barrier(world)
     launches = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p) - l0
+    kname = {"greedy": hs.hs_last_kernel(plan_g) if do_g else None, "presto": hs.hs_last_kernel(plan_p) if do_p else None}
     total_ms = evs[0][0].elapsed_time(evs[-1][2])          # device time of exactly K steps
     g_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     p_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
@@ -292,6 +322,9 @@ def run_cuda(args):
         hx.copy_(x)
         hsnr = torch.empty((S, N), dtype=torch.float32, pin_memory=True)
         hbh = torch.empty((S, N), dtype=torch.int32, pin_memory=True)
+        both = do_g and do_p and args.greedy_flags == 0 and args.presto_flags == 0
+        hsnr2 = torch.empty((S, N), dtype=torch.float32, pin_memory=True) if both else None
+        hbh2 = torch.empty((S, N), dtype=torch.int32, pin_memory=True) if both else None
         e_steps = max(1, min(args.steps, 5))
 
         hib = None
@@ -300,6 +333,9 @@ def run_cuda(args):
             hib.copy_(ib)
 
         def e2e_step():
+            if both:            # one upload of the spectra, both forms computed from it
+                hs.hs_run_both_host(plan_g, hx, hib, mu_g, sg_g, hsnr, hbh, None, mu_p, sg_p, hsnr2, hbh2)
+                return
             if do_g:
                 hs.hs_run_greedy_host(plan_g, hx, hib, mu_g, sg_g, hsnr, hbh, None)
             if do_p:
@@ -313,11 +349,12 @@ def run_cuda(args):
         barrier(world)
         dt = max_over_ranks(time.perf_counter() - t0, dev)
         e2e = {"value": bins_step * e_steps / dt, "unit": UNIT, "steps": e_steps,
-               "h2d_bytes_per_step": n_forms * S * N * 4 * (2 if ib is not None else 1),
+               "h2d_bytes_per_step": (1 if both else n_forms) * S * N * 4 * (2 if ib is not None else 1),
                "d2h_bytes_per_step": n_forms * S * N * 8,
                "ms_per_step": 1e3 * dt / e_steps,
-               "note": "hs_run_greedy_host + hs_run_presto_host, pinned host buffers, per rank; PCIe-bound"}
-        del hx, hsnr, hbh, hib
+               "note": ("hs_run_both_host (one upload, both forms)" if both else "hs_run_greedy_host / hs_run_presto_host") +
+                       ", pinned host buffers, per rank; PCIe-bound"}
+        del hx, hsnr, hbh, hib, hsnr2, hbh2
 
     # ---- NEXT-3: candidate list of the greedy outputs (one streaming pass; outside the step) ----
     cand = None
@@ -345,17 +382,44 @@ def run_cuda(args):
         a = alg_bytes / (ms * 1e-3) / 1e9
         return a, a / peak
 
+    ncu = _load_json(NCU_KERNELS_JSON)
+    mm = _load_json(MACHINE_MODEL_JSON)
+    full_cfg3 = (w.name == "cfg3" and S == w.n_spectra and H == w.H and ib is None
+                 and not args.greedy_flags and not args.presto_flags)
+
+    def evidence(form):
+        """Committed ncu counters of the kernel that actually ran (cfg3 captures only); None when there are none."""
+        rec = ncu.get(kname[form] or "", None) if full_cfg3 else None
+        return rec if isinstance(rec, dict) else None
+
+    def second(form, ms):
+        """The on-chip ceiling beside the HBM one: L2 -> SM sector bytes of the launch over the measured L2 -> SM rate."""
+        rec = evidence(form)
+        l2 = mm.get("l2_to_sm_gbs")
+        if rec is None or not l2 or not rec.get("l2_to_sm_sector_bytes"):
+            return None
+        floor_ms = rec["l2_to_sm_sector_bytes"] / (l2 * 1e9) * 1e3
+        return {"l2_to_sm_gbs": l2, "sector_bytes_per_launch": rec["l2_to_sm_sector_bytes"],
+                "ceiling_ms": floor_ms, "frac_of_ceiling": floor_ms / ms, "source": mm.get("source"), "capture": rec.get("capture")}
+
+    def per_kernel(form, ms):
+        rec = evidence(form)
+        return {"kernel": kname[form], "launch_ms": ms, "achieved": roof(ms)[0], "frac": roof(ms)[1],
+                "gbins_per_s": S * N / ms / 1e6,
+                "traffic": (rec["dram_bytes_read"] + rec["dram_bytes_write"]) if rec else None,
+                "secondary_ceiling": second(form, ms)}
+
     a, fr = roof(dom_ms)
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": a, "peak": peak, "unit": "GB/s", "frac": fr,
-                "traffic": NCU_TRAFFIC_BYTES[dom] if default_run else None, "peak_source": peak_src,
+    dom_rec = evidence(dom)
+    roofline = {"bound": "hbm", "kernel": dom, "kernel_name": kname[dom], "achieved": a, "peak": peak, "unit": "GB/s", "frac": fr,
+                "traffic": (dom_rec["dram_bytes_read"] + dom_rec["dram_bytes_write"]) if dom_rec else None,
+                "traffic_source": dom_rec.get("capture") if dom_rec else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": dom_ms,
-                "per_kernel": {}}
+                "secondary_ceiling": second(dom, dom_ms), "per_kernel": {}}
     if do_g:
-        roofline["per_kernel"]["greedy"] = {"launch_ms": g_ms, "achieved": roof(g_ms)[0], "frac": roof(g_ms)[1],
-                                            "gbins_per_s": S * N / g_ms / 1e6}
+        roofline["per_kernel"]["greedy"] = per_kernel("greedy", g_ms)
     if do_p:
-        roofline["per_kernel"]["presto"] = {"launch_ms": p_ms, "achieved": roof(p_ms)[0], "frac": roof(p_ms)[1],
-                                            "gbins_per_s": S * N / p_ms / 1e6}
+        roofline["per_kernel"]["presto"] = per_kernel("presto", p_ms)
 
     cpu = None
     if rank == 0 and not args.no_cpu:
@@ -390,6 +454,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
     return run_cuda(args)
 
 

@@ -39,9 +39,12 @@
  *        snr = (sum - mu[H'-1]) / sigma[H'-1];  if snr > best { best = snr; best_h = H' }
  *   With d_inv_baseline != NULL every x[b] above is replaced by the fp32 product
  *   x[b] * inv_baseline[b] (spectrum whitening supplied by the caller).
- *   Sums are accumulated in fp32 in the order written above (for the ALL_HARMONICS variants the terms of
- *   one H' may instead be grouped by reduced fraction h/H', each group in increasing h, groups in
- *   increasing denominator); the SNR is formed as
+ *   Sums are accumulated in fp32.  Greedy: in the order written above.  PRESTO (Alg. 1): the harmonic sets are
+ *   nested (the terms of H' are those of H'/2 plus the new fractions h/H' with h/2 odd), and the default kernel
+ *   forms S_{H'} = S_{H'/2} + (the new terms of H' summed first, by increasing level-local order) -- a different
+ *   fp32 association from the loop above, inside the stated tolerance; the coverage kernel adds in the written
+ *   order.  ALL_HARMONICS variants: the terms of one H' may be grouped by reduced fraction h/H', each group in
+ *   increasing h, groups in increasing denominator.  The SNR is formed as
  *   fma(sum, 1/sigma, -mu/sigma) in fp32, both constants rounded once on the host.  Non-finite
  *   inputs give unspecified results.
  *
@@ -86,15 +89,7 @@ enum {
     HS_GREEDY_NO_FUND_SELECT = 1u << 0, /* order 1 takes x[n] without comparing with x[n+1] (PAPER.md:260 is optional) */
     HS_GREEDY_NO_DRIFT       = 1u << 1, /* simple harmonic sum, eq. 3: the drift stays 0 */
     HS_PRESTO_ALL_HARMONICS  = 1u << 2, /* PRESTO_all: sum every harmonic 1..H' */
-    HS_PRESTO_ALL_ORDERS     = 1u << 3, /* with ALL_HARMONICS = PRESTO+: every H' = 1..H */
-    /* tuning knob, not semantics: bits 16..23 select a kernel variant (0 = the library's choice);
-       every variant computes the results defined above */
-    HS_TUNE_SHIFT            = 16,
-    HS_TUNE_MASK             = 0xFFu << 16,
-    /* tuning knob: bits 24..27 = spectra per launch group of the two-pass greedy kernels (0 = the
-       library's choice, sized so that the group stays L2-resident) */
-    HS_CHUNK_SHIFT           = 24,
-    HS_CHUNK_MASK            = 0xFu << 24
+    HS_PRESTO_ALL_ORDERS     = 1u << 3  /* with ALL_HARMONICS = PRESTO+: every H' = 1..H */
 };
 
 /* Create a plan for a batch shape.
@@ -106,9 +101,11 @@ enum {
  *   n_fund     outputs are computed for n < n_fund (0 = n_bins); <= n_bins
  *   flags      OR of the enum above; HS_PRESTO_ALL_ORDERS requires HS_PRESTO_ALL_HARMONICS
  *   device     CUDA device ordinal
- * The plan owns only small internal state (device properties, launch geometry, a comparison-mask
- * scratch of one bit per bin for the few spectra the greedy mask variants keep in flight, and --
- * once a *_host entry point has been used -- its staging buffers and streams). */
+ * The plan owns only small internal host state (shape, device properties); hs_plan allocates nothing on
+ * the device and does not synchronise.  Once a *_host entry point has been used the plan also owns that
+ * path's device staging buffers and streams.  n_spectra has no limit other than memory.
+ * Every entry point that takes a plan runs on the plan's device whatever device is current, and leaves
+ * the caller's current device unchanged. */
 hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
                   int64_t in_stride, int64_t out_stride, int64_t n_fund,
                   uint32_t flags, int32_t device);
@@ -142,6 +139,14 @@ hs_status hs_run_presto_host(hs_plan_t plan, const float* h_spectra, const float
                              const float* mu, const float* sigma,
                              float* h_snr, int32_t* h_best_h);
 
+/* Both forms from ONE upload of the spectra: greedy (outputs h_snr_greedy, h_best_h_greedy, optional h_path) and
+ * PRESTO (h_snr_presto, h_best_h_presto) with their own statistics; otherwise as the two calls above. */
+hs_status hs_run_both_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline,
+                           const float* mu_greedy, const float* sigma_greedy,
+                           float* h_snr_greedy, int32_t* h_best_h_greedy, uint32_t* h_path,
+                           const float* mu_presto, const float* sigma_presto,
+                           float* h_snr_presto, int32_t* h_best_h_presto);
+
 /* One detection (reading R11 of DESIGN.md: a bin whose maximum SNR reaches the threshold). */
 typedef struct {
     int32_t spectrum;   /* row s of the batch */
@@ -160,8 +165,17 @@ typedef struct {
 hs_status hs_find_candidates(hs_plan_t plan, const float* d_snr, const int32_t* d_best_h, float threshold,
                              hs_candidate* d_out, int64_t capacity, uint64_t* d_count, void* cuda_stream);
 
+/* UNSTABLE, diagnostics only (not part of the method's interface; values may change between versions):
+ * selects a kernel variant for the plan's later runs.  0 = the library's choice; 255 = the plain
+ * one-thread-per-bin coverage kernels.  Every variant computes the results defined above. */
+hs_status hs_plan_set_tuning(hs_plan_t plan, uint32_t variant);
+
 /* Number of kernels this plan has launched so far (for bench.py's gpu_launches). */
 int64_t hs_launch_count(hs_plan_t plan);
+
+/* Name of the kernel variant the plan launched last ("" before the first run): bench.py keys its committed
+ * ncu evidence (profiles/) by this name.  Static string. */
+const char* hs_last_kernel(hs_plan_t plan);
 
 /* Release the plan and everything it owns.  NULL is accepted. */
 hs_status hs_destroy(hs_plan_t plan);

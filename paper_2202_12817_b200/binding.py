@@ -22,10 +22,11 @@ HS_GREEDY_NO_FUND_SELECT = 1 << 0
 HS_GREEDY_NO_DRIFT = 1 << 1
 HS_PRESTO_ALL_HARMONICS = 1 << 2
 HS_PRESTO_ALL_ORDERS = 1 << 3
-HS_TUNE_SHIFT = 16
+HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
-EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_find_candidates",
-           "hs_launch_count", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
+EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
+           "hs_find_candidates", "hs_plan_set_tuning",
+           "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
 class HsError(RuntimeError):
@@ -61,10 +62,16 @@ def load() -> ctypes.CDLL:
     lib.hs_run_greedy_host.restype = ctypes.c_int
     lib.hs_run_presto_host.argtypes = [vp, vp, vp, fp, fp, vp, vp]
     lib.hs_run_presto_host.restype = ctypes.c_int
+    lib.hs_run_both_host.argtypes = [vp, vp, vp, fp, fp, vp, vp, vp, fp, fp, vp, vp]
+    lib.hs_run_both_host.restype = ctypes.c_int
+    lib.hs_plan_set_tuning.argtypes = [vp, u32]
+    lib.hs_plan_set_tuning.restype = ctypes.c_int
     lib.hs_find_candidates.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp, vp]
     lib.hs_find_candidates.restype = ctypes.c_int
     lib.hs_launch_count.argtypes = [vp]
     lib.hs_launch_count.restype = i64
+    lib.hs_last_kernel.argtypes = [vp]
+    lib.hs_last_kernel.restype = ctypes.c_char_p
     lib.hs_destroy.argtypes = [vp]
     lib.hs_destroy.restype = ctypes.c_int
     lib.hs_status_string.argtypes = [ctypes.c_int]
@@ -151,6 +158,19 @@ def hs_run_presto_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best
            "hs_run_presto_host")
 
 
+def hs_run_both_host(plan, h_spectra, h_inv_baseline, mu_greedy, sigma_greedy, h_snr_greedy, h_best_h_greedy, h_path,
+                     mu_presto, sigma_presto, h_snr_presto, h_best_h_presto) -> None:
+    lib = load()
+    _check(lib.hs_run_both_host(plan, _hptr(h_spectra, torch.float32, "h_spectra"),
+                                _hptr(h_inv_baseline, torch.float32, "h_inv_baseline"),
+                                _farr(mu_greedy), _farr(sigma_greedy),
+                                _hptr(h_snr_greedy, torch.float32, "h_snr_greedy"),
+                                _hptr(h_best_h_greedy, torch.int32, "h_best_h_greedy"), _hptr(h_path, torch.int32, "h_path"),
+                                _farr(mu_presto), _farr(sigma_presto),
+                                _hptr(h_snr_presto, torch.float32, "h_snr_presto"),
+                                _hptr(h_best_h_presto, torch.int32, "h_best_h_presto")), "hs_run_both_host")
+
+
 def hs_find_candidates(plan, d_snr: torch.Tensor, d_best_h: torch.Tensor, threshold: float,
                        d_out: Optional[torch.Tensor], d_count: torch.Tensor, stream: Optional[int] = None) -> None:
     """d_out: int32 CUDA tensor [capacity, 4] (rows = hs_candidate: spectrum, bin, snr bits, best_h) or None;
@@ -166,8 +186,16 @@ def hs_find_candidates(plan, d_snr: torch.Tensor, d_best_h: torch.Tensor, thresh
                                   _dptr(d_count, torch.int64, "d_count"), stream), "hs_find_candidates")
 
 
+def hs_plan_set_tuning(plan, variant: int) -> None:
+    _check(load().hs_plan_set_tuning(plan, int(variant)), "hs_plan_set_tuning")
+
+
 def hs_launch_count(plan) -> int:
     return int(load().hs_launch_count(plan))
+
+
+def hs_last_kernel(plan) -> str:
+    return load().hs_last_kernel(plan).decode()
 
 
 def hs_destroy(plan) -> None:

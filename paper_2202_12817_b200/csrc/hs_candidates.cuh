@@ -17,7 +17,7 @@ struct HsCandidate {       // == hs_candidate (hs.h)
 
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
-hs_candidates_kernel(const float* __restrict__ snr, const int* __restrict__ best_h, long long out_stride, int n_fund,
+hs_candidates_kernel(const float* __restrict__ snr, const int* __restrict__ best_h, long long out_stride, int n_fund, int s0,
                      float threshold, HsCandidate* __restrict__ out, unsigned long long capacity,
                      unsigned long long* __restrict__ count) {
     const int s = blockIdx.y;
@@ -59,7 +59,7 @@ hs_candidates_kernel(const float* __restrict__ snr, const int* __restrict__ best
                 if (hit & (1u << e)) {
                     if (pos < capacity) {
                         HsCandidate cand;
-                        cand.spectrum = s; cand.bin = n + e; cand.snr = v[e]; cand.best_h = __ldg(brow + n + e);
+                        cand.spectrum = s0 + s; cand.bin = n + e; cand.snr = v[e]; cand.best_h = __ldg(brow + n + e);
                         *reinterpret_cast<int4*>(out + pos) = *reinterpret_cast<const int4*>(&cand);
                     }
                     ++pos;

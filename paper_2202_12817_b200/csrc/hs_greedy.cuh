@@ -1,5 +1,5 @@
 // Tuned greedy harmonic sum (Alg. 2) for the common configuration:
-// no per-bin baseline, drift tracking on, in-row indices < 2^31.
+// drift tracking on (or off: the simple sum), in-row indices < 2^31.
 //
 // Mapping: a CTA owns a tile of R*BLOCK consecutive fundamentals of
 // one spectrum; thread t runs R independent chains, chain j on fundamental f0 + j*BLOCK + t, so
@@ -9,21 +9,48 @@
 // spectrum-major (blockIdx.y = spectrum) so a spectrum is swept while it is L2-resident:
 // every bin b is re-read at order h by the fundamentals near b/h.
 // The R chains give the memory system R independent dependent-load chains per thread.
+//
+// Tile order inside a spectrum (MIX): consecutive CTAs take tiles from 16 equally wide bands of
+// fundamentals in turn (8 of every 16 from the one-order top band, which only streams HBM; one from
+// the lowest sixteenth, which gathers all H orders out of L2), so that every SM holds a mix of
+// HBM-bound and L2-bound tiles at any moment instead of running the two kinds one after the other.
+//
+// Addressing: the chain keeps the BYTE offset of x[m] inside the row in one 32-bit register
+// (4 m < 2^33 does not fit: the offset is kept in ELEMENTS and the load address is formed by one
+// IMAD.WIDE from the row pointer, which is materialised once).
 #pragma once
 #include "hs_common.cuh"
 
+namespace hs_greedy {
+constexpr int NBAND = 16;
+// tile visited by CTA i of a spectrum with nt tiles: band i % 16, position i / 16 inside the band
+__device__ __forceinline__ int mixed_tile(int i, int nt) {
+    const int per = (nt + NBAND - 1) / NBAND;
+    return (i % NBAND) * per + i / NBAND;               // may be >= nt: the CTA has nothing to do
+}
+__host__ __device__ constexpr int mixed_grid(int nt) { return NBAND * ((nt + NBAND - 1) / NBAND); }
+}  // namespace hs_greedy
+
 // HAS_BASE: every x[b] is the fp32 product x[b] * inv_baseline[b] (reading R13; cfg4's whitening multiplier).
 // DRIFT = false: the simple harmonic sum (eq. 3; HS_GREEDY_NO_DRIFT): the second bin is never read.
-template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true>
+template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true, bool MIX = true>
 __global__ void __launch_bounds__(BLOCK, (R == 4) ? 1536 / BLOCK : 1)
 hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
     const int s = blockIdx.y;
     const int N = (int)sh.n_bins;
     const int last = N - 1;
     const int n_fund = (int)sh.n_fund;
-    const int f0 = blockIdx.x * (BLOCK * R);
-    const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
-    const float* __restrict__ ib = HAS_BASE ? io.inv_base + (long long)s * sh.in_stride : nullptr;
+    int tile = blockIdx.x;
+    if (MIX) {
+        const int nt = (n_fund + BLOCK * R - 1) / (BLOCK * R);
+        tile = hs_greedy::mixed_tile(blockIdx.x, nt);
+        if (tile >= nt) return;
+    }
+    const int f0 = tile * (BLOCK * R);
+    const float* x = io.x + (long long)s * sh.in_stride;
+    const float* ib = HAS_BASE ? io.inv_base + (long long)s * sh.in_stride : nullptr;
+    asm volatile("" : "+l"(x));                                  // one materialised row pointer for all the loads
+    if (HAS_BASE) asm volatile("" : "+l"(ib));
 
     // Orders 1..h_safe need no band-edge test for any fundamental of the tile:
     // m + 1 = h n + d + 1 <= h (n + 1) + 1 <= last.   Orders above h_top are dead for all of them.
@@ -38,7 +65,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     if (!HAS_BASE && h_top == 1 && f0 + BLOCK * R <= n_fund && f0 + BLOCK * R + 1 <= N && (BLOCK * R) % 128 == 0) {
         if (threadIdx.x < BLOCK * R / 4) {                          // whole warps: BLOCK R / 4 is a multiple of 32
             const int n0 = f0 + 4 * threadIdx.x;
-            const float4 v = __ldg(reinterpret_cast<const float4*>(x + n0));
+            const float4 v = __ldcs(reinterpret_cast<const float4*>(x + n0));      // last use of these bins: evict first
             float nxt = __shfl_down_sync(0xffffffffu, v.x, 1);
             if ((threadIdx.x & 31) == 31) nxt = __ldg(x + n0 + 4);
             const float e[5] = {v.x, v.y, v.z, v.w, nxt};
@@ -58,42 +85,43 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         return;
     }
 
-    int n[R], d[R], hn[R], bh[R];
+    // chain state: m = element offset of x[h n + d] (advanced by n per order, by 1 per shift)
+    unsigned n[R], m[R];
+    int bh[R];
     float sum[R], best[R];
     unsigned path[R];
-#pragma unroll
-    for (int j = 0; j < R; ++j) {
-        n[j] = f0 + j * BLOCK + threadIdx.x;
-        d[j] = 0; hn[j] = 0; bh[j] = 0; sum[j] = 0.f; best[j] = HS_NEG_INF; path[j] = 0;
-    }
     bool live[R];
 #pragma unroll
-    for (int j = 0; j < R; ++j) live[j] = n[j] < n_fund;
-#pragma unroll
-    for (int j = 0; j < R; ++j) if (!live[j]) n[j] = n_hi;       // clamp: harmless duplicate work, no OOB
+    for (int j = 0; j < R; ++j) {
+        const int nj = f0 + j * BLOCK + threadIdx.x;
+        live[j] = nj < n_fund;
+        n[j] = live[j] ? nj : n_hi;                              // clamp: harmless duplicate work, no OOB
+        m[j] = 0; bh[j] = 0; sum[j] = 0.f; best[j] = HS_NEG_INF; path[j] = 0;
+    }
 
     int h = 1;
     // ---- unchecked orders ----
+#pragma unroll 2
     for (; h <= h_safe; ++h) {
         const float nmis = st.nmis[h - 1], is = st.inv_sigma[h - 1];
         float a[R], b[R];
 #pragma unroll
         for (int j = 0; j < R; ++j) {
-            hn[j] += n[j];
-            const int m = hn[j] + d[j];
-            a[j] = __ldg(x + m);
-            if (HAS_BASE) a[j] = __fmul_rn(a[j], __ldg(ib + m));
+            m[j] += n[j];
+            const float* p = x + m[j];
+            a[j] = __ldg(p);
+            if (HAS_BASE) a[j] = __fmul_rn(a[j], __ldg(ib + m[j]));
             b[j] = HS_NEG_INF;
             if (DRIFT) {
-                b[j] = __ldg(x + m + 1);
-                if (HAS_BASE) b[j] = __fmul_rn(b[j], __ldg(ib + m + 1));
+                b[j] = __ldg(p + 1);
+                if (HAS_BASE) b[j] = __fmul_rn(b[j], __ldg(ib + m[j] + 1));
             }
         }
 #pragma unroll
         for (int j = 0; j < R; ++j) {
             bool shift = b[j] > a[j];
             if (!FUND_SELECT) shift = shift && (h != 1);
-            d[j] += shift;
+            m[j] += shift;
             sum[j] = __fadd_rn(sum[j], shift ? b[j] : a[j]);
             if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
             const float snr = hs_snr(sum[j], nmis, is);
@@ -108,19 +136,18 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         const float nmis = st.nmis[h - 1], is = st.inv_sigma[h - 1];
 #pragma unroll
         for (int j = 0; j < R; ++j) {
-            hn[j] += n[j];
-            const int m = hn[j] + d[j];
-            alive[j] = alive[j] && (m <= last);
+            m[j] += n[j];                                        // < N + 32 n: no wrap (hs_api.cu limits N)
+            alive[j] = alive[j] && (m[j] <= (unsigned)last);
             if (alive[j]) {
-                float a = __ldg(x + m);
-                if (HAS_BASE) a = __fmul_rn(a, __ldg(ib + m));
+                float a = __ldg(x + m[j]);
+                if (HAS_BASE) a = __fmul_rn(a, __ldg(ib + m[j]));
                 float b = HS_NEG_INF;
-                if (DRIFT && m + 1 <= last && (FUND_SELECT || h != 1)) {
-                    b = __ldg(x + m + 1);
-                    if (HAS_BASE) b = __fmul_rn(b, __ldg(ib + m + 1));
+                if (DRIFT && m[j] + 1 <= (unsigned)last && (FUND_SELECT || h != 1)) {
+                    b = __ldg(x + m[j] + 1);
+                    if (HAS_BASE) b = __fmul_rn(b, __ldg(ib + m[j] + 1));
                 }
                 const bool shift = b > a;
-                d[j] += shift;
+                m[j] += shift;
                 sum[j] = __fadd_rn(sum[j], shift ? b : a);
                 if (WANT_PATH) path[j] |= (unsigned)shift << (h - 1);
                 const float snr = hs_snr(sum[j], nmis, is);

@@ -9,7 +9,7 @@ from paper_2202_12817_b200 import inputs
 pytestmark = pytest.mark.gpu
 
 NO_FUND_SELECT, NO_DRIFT, ALL_HARMONICS, ALL_ORDERS = 1, 2, 4, 8
-GENERIC = 255 << 16          # HS_TUNE value that forces the generic kernels
+GENERIC = 255                # hs_plan_set_tuning value that forces the coverage kernels
 
 
 @pytest.fixture(scope="module")
@@ -20,7 +20,7 @@ def hs():
     return binding
 
 
-def run_greedy(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, want_path=True, in_stride=0, out_stride=0):
+def run_greedy(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, want_path=True, in_stride=0, out_stride=0, tune=0):
     x = torch.as_tensor(x)
     if x.ndim == 1:
         x = x[None, :]
@@ -39,6 +39,7 @@ def run_greedy(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, want_path
     path = torch.full((S, ostr), -7, dtype=torch.int32, device="cuda") if want_path else None
     plan = hs.hs_plan(N, S, H, istr, ostr, n_fund, flags, 0)
     try:
+        hs.hs_plan_set_tuning(plan, tune)
         hs.hs_run_greedy(plan, dx, db, mu, sg, snr, bh, path)
         torch.cuda.synchronize()
         assert hs.hs_launch_count(plan) >= 1
@@ -50,7 +51,7 @@ def run_greedy(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, want_path
             path[:, :nf].cpu().numpy() if want_path else None)
 
 
-def run_presto(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, in_stride=0, out_stride=0):
+def run_presto(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, in_stride=0, out_stride=0, tune=0):
     x = torch.as_tensor(x)
     if x.ndim == 1:
         x = x[None, :]
@@ -68,6 +69,7 @@ def run_presto(hs, x, H, mu, sg, flags=0, inv_baseline=None, n_fund=0, in_stride
     bh = torch.full((S, ostr), -7, dtype=torch.int32, device="cuda")
     plan = hs.hs_plan(N, S, H, istr, ostr, n_fund, flags, 0)
     try:
+        hs.hs_plan_set_tuning(plan, tune)
         hs.hs_run_presto(plan, dx, db, mu, sg, snr, bh)
         torch.cuda.synchronize()
     finally:
@@ -89,9 +91,9 @@ def _int_stats(H):
 SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (2, 1 << 17)]
 
 
-# tune word: kernel variant in bits 16..23 (20..27 = two-pass comparison-mask kernels), spectra per launch
-# group in bits 24..27
-GREEDY_TUNES = [0, 1, 3, 4, 6, 8, 255, 20, 22 | (2 << 8), 24 | (1 << 8), 25, 26, 27 | (3 << 8), 29]
+# hs_plan_set_tuning values: 0 = the library's choice, 255 = coverage kernels, others = alternative tile shapes
+GREEDY_TUNES = [0, 3, 255]
+PRESTO_TUNES = [0, 31, 255]
 
 
 @pytest.mark.parametrize("tune", GREEDY_TUNES)
@@ -102,32 +104,32 @@ def test_greedy_exact_integer(hs, oracle_mod, tune, H):
         x = inputs.integer_spectra(100 + N, S, N, 255).numpy()
         for flags in (0, NO_FUND_SELECT):
             s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags)
-            s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16))
+            s, b, p = run_greedy(hs, x, H, mu, sg, flags, tune=tune)
             assert np.array_equal(p.view(np.uint32), p_ref), (S, N, flags)
             assert np.array_equal(b, b_ref), (S, N, flags)
             assert np.array_equal(s.astype(np.float64), s_ref), (S, N, flags)
 
 
-@pytest.mark.parametrize("tune", [0, 1, 3, 5, 6, 10, 11, 12, 13, 14, 15, 16, 30, 31, 33, 35, 50, 255])
+@pytest.mark.parametrize("tune", PRESTO_TUNES)
 @pytest.mark.parametrize("H", [1, 2, 4, 8, 13, 16, 32])
 def test_presto_exact_integer(hs, oracle_mod, tune, H):
     mu, sg = _int_stats(H)
     for S, N in SHAPES:
         x = inputs.integer_spectra(200 + N, S, N, 255).numpy()
         s_ref, b_ref = oracle_mod.presto(x, H, mu, sg)
-        s, b = run_presto(hs, x, H, mu, sg, tune << 16)
+        s, b = run_presto(hs, x, H, mu, sg, tune=tune)
         assert np.array_equal(b, b_ref), (S, N)
         assert np.array_equal(s.astype(np.float64), s_ref), (S, N)
 
 
-@pytest.mark.parametrize("tune", [0, 1, 255])
+@pytest.mark.parametrize("tune", [0, 255])
 @pytest.mark.parametrize("flags", [NO_DRIFT, NO_DRIFT | NO_FUND_SELECT])
 def test_simple_hs_exact_integer(hs, oracle_mod, flags, tune):
     H = 16
     mu, sg = _int_stats(H)
     x = inputs.integer_spectra(7, 3, 5003, 255).numpy()
     s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags)
-    s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16))
+    s, b, p = run_greedy(hs, x, H, mu, sg, flags, tune=tune)
     assert np.all(p == 0) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
 
 
@@ -139,7 +141,7 @@ def test_presto_variants_exact_integer(hs, oracle_mod, flags, H, tune):
     for S, N in ((2, 6007), (1, 2), (3, 257), (2, 70001)):
         x = inputs.integer_spectra(8 + N, S, N, 255).numpy()
         s_ref, b_ref = oracle_mod.presto(x, H, mu, sg, flags)
-        s, b = run_presto(hs, x, H, mu, sg, flags | (tune << 16))
+        s, b = run_presto(hs, x, H, mu, sg, flags, tune=tune)
         assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref), (S, N)
 
 
@@ -150,10 +152,10 @@ def test_strides_and_n_fund(hs, oracle_mod):
     x = inputs.integer_spectra(9, S, N, 255).numpy()
     for tune in (0, 255):
         s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, 0, n_fund=1234)
-        s, b, p = run_greedy(hs, x, H, mu, sg, tune << 16, n_fund=1234, in_stride=5008, out_stride=1300)
+        s, b, p = run_greedy(hs, x, H, mu, sg, 0, n_fund=1234, in_stride=5008, out_stride=1300, tune=tune)
         assert np.array_equal(p.view(np.uint32), p_ref) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
         q_ref, c_ref = oracle_mod.presto(x, H, mu, sg, 0, n_fund=777)
-        q, c = run_presto(hs, x, H, mu, sg, tune << 16, n_fund=777, in_stride=5120, out_stride=780)
+        q, c = run_presto(hs, x, H, mu, sg, 0, n_fund=777, in_stride=5120, out_stride=780, tune=tune)
         assert np.array_equal(c, c_ref) and np.array_equal(q.astype(np.float64), q_ref)
     # without the optional path output
     s2, b2, _ = run_greedy(hs, x, H, mu, sg, 0, want_path=False)
@@ -170,13 +172,13 @@ def test_cfg1_both_variants(hs, oracle_mod, tune):
     w = inputs.workload("cfg1")
     x = inputs.generate(w).numpy()
     mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", w.H))
-    s, b, p = run_greedy(hs, x, w.H, mu, sg, tune << 16)
+    s, b, p = run_greedy(hs, x, w.H, mu, sg, tune=tune)
     r = check_greedy(oracle_mod, x, w.H, mu, sg, 0, s, b, p, T=10.0)
     # the injected pulsar (r = 1000.5) is detected at its fundamental
     top = int(np.argmax(s[0]))
     assert top in (1000, 1001) and s[0, top] > 10.0
     mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", w.H))
-    s, b = run_presto(hs, x, w.H, mu, sg, tune << 16)
+    s, b = run_presto(hs, x, w.H, mu, sg, tune=tune)
     check_presto(oracle_mod, x, w.H, mu, sg, 0, s, b, T=10.0)
     assert r["bh_mismatch"] < 10
 
@@ -223,14 +225,14 @@ def test_inv_baseline_red_noise(hs, oracle_mod):
     for tune in (0, 3, 255):                 # tuned tile kernels with the multiplier, and the generic kernel
         for flags, fs in ((0, True), (NO_FUND_SELECT, False)):
             mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H, fs))
-            s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16), inv_baseline=ib)
+            s, b, p = run_greedy(hs, x, H, mu, sg, flags, inv_baseline=ib, tune=tune)
             check_greedy(oracle_mod, x, H, mu, sg, flags, s, b, p, inv_baseline=ib, T=10.0)
     mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
     s, b = run_presto(hs, x, H, mu, sg, 0, inv_baseline=ib)
     check_presto(oracle_mod, x, H, mu, sg, 0, s, b, inv_baseline=ib, T=10.0)
 
 
-@pytest.mark.parametrize("tune", [0, 1, 6, 255])
+@pytest.mark.parametrize("tune", [0, 3, 255])
 def test_inv_baseline_exact_integer(hs, oracle_mod, tune):
     """Integer powers times power-of-two multipliers: every product, sum and SNR is exact (pin P7 with R13)."""
     H = 32
@@ -241,7 +243,7 @@ def test_inv_baseline_exact_integer(hs, oracle_mod, tune):
     ib = (2.0 ** rng.integers(-1, 3, size=(S, N))).astype(np.float32)
     for flags in (0, NO_FUND_SELECT):
         s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, flags, inv_baseline=ib)
-        s, b, p = run_greedy(hs, x, H, mu, sg, flags | (tune << 16), inv_baseline=ib)
+        s, b, p = run_greedy(hs, x, H, mu, sg, flags, inv_baseline=ib, tune=tune)
         assert np.array_equal(p.view(np.uint32), p_ref) and np.array_equal(b, b_ref)
         assert np.array_equal(s.astype(np.float64), s_ref)
 
