@@ -462,21 +462,31 @@ def _sample_bins(N, rng, k=6000):
     return np.unique(np.concatenate([edges, rng.integers(0, N, size=k), rng.integers(0, max(1, N // 32), size=k)]))
 
 
-def test_maximum_sizes_sampled(hs, oracle_mod):
-    """Largest rows the fast paths accept: greedy tile kernel at N = 2^30 + 7 (32-bit h n close to its limit), PRESTO
-    rows kernel at N = 2^26 - 70 (32 N just below 2^31).  Exact-integer spectra, so sampled outputs must equal the
-    oracle's bit for bit (the oracle computes the sampled bins one by one)."""
+@pytest.mark.parametrize("kind,N,kernel", [
+    ("greedy", (1 << 30) + 7, "hs_greedy_tile_kernel"),            # 32-bit h n close to its limit
+    ("presto", (1 << 26) - 70, "hs_presto_rows_kernel"),           # 32 N just below 2^31
+    ("presto", (1 << 26) + 8, "hs_presto_generic_kernel"),         # just past the rows kernel's limit
+    ("greedy", (1 << 31) - (1 << 17), "hs_greedy_tile_kernel"),    # the last N the tile kernel takes
+    ("greedy", (1 << 31) - 64, "hs_greedy_generic_kernel"),        # the largest N hs_plan accepts: 64-bit offsets
+])
+def test_maximum_sizes_sampled(hs, oracle_mod, kind, N, kernel):
+    """Largest rows the fast paths accept and the first sizes past each fast-path limit (which kernel ran is
+    asserted through hs_last_kernel).  Exact-integer spectra, so sampled outputs must equal the oracle's bit for
+    bit (the oracle computes the sampled bins one by one)."""
     free, _ = torch.cuda.mem_get_info()
     if free < 30 * (1 << 30):
         pytest.skip("needs 30 GiB of device memory")
     H = 32
     mu, sg = _int_stats(H)
     rng = np.random.default_rng(11)
-    for kind, N in (("greedy", (1 << 30) + 7), ("presto", (1 << 26) - 70)):
+    if True:
         g = torch.Generator(device="cuda"); g.manual_seed(5)
         istr = (N + 3) & ~3
         x = torch.zeros((1, istr), dtype=torch.float32, device="cuda")
-        x[0, :N] = torch.randint(0, 256, (N,), generator=g, device="cuda", dtype=torch.int32).to(torch.float32)
+        step = 1 << 28                                             # in pieces: no 8 GiB temporaries
+        for a in range(0, N, step):
+            b = min(N, a + step)
+            x[0, a:b] = torch.randint(0, 256, (b - a,), generator=g, device="cuda", dtype=torch.int32).to(torch.float32)
         snr = torch.empty((1, istr), dtype=torch.float32, device="cuda")
         bh = torch.empty((1, istr), dtype=torch.int32, device="cuda")
         path = torch.empty((1, istr), dtype=torch.int32, device="cuda") if kind == "greedy" else None
@@ -487,6 +497,7 @@ def test_maximum_sizes_sampled(hs, oracle_mod):
             else:
                 hs.hs_run_presto(plan, x, None, mu, sg, snr, bh)
             torch.cuda.synchronize()
+            assert hs.hs_last_kernel(plan).startswith(kernel), hs.hs_last_kernel(plan)
         finally:
             hs.hs_destroy(plan)
         bins = _sample_bins(N, rng)
@@ -502,3 +513,105 @@ def test_maximum_sizes_sampled(hs, oracle_mod):
         assert np.array_equal(snr[0, idx].cpu().numpy().astype(np.float64), ref["snr"])
         del x, snr, bh, path, xh
         torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------------------------------
+# All rows of the headline batch: tuned kernels against the coverage kernels (which the oracle vouches for
+# element by element in the tests above), so that the oracle-checked rows vouch for the rest
+# ------------------------------------------------------------------------------------------
+def test_cfg3_all_rows_tuned_vs_generic(hs, oracle_mod):
+    """cfg3 content, all 256 rows, one launch each.  Greedy: the tile kernel and hs_greedy_generic_kernel add the
+    same fp32 terms in the same order, so snr, best_h and path must be equal bit for bit.  PRESTO: the rows kernel
+    adds level by level (hs.h "Precision"), so snr agrees within the fp32 accumulation bound and best_h may differ
+    only where the two maxima are within that bound; on exact-integer spectra of the same shape it is bit for bit."""
+    w = inputs.workload("cfg3")
+    S, N, H = w.n_spectra, w.n_bins, w.H
+    free, _ = torch.cuda.mem_get_info()
+    if free < 32 * (1 << 30):
+        pytest.skip("needs 32 GiB of device memory")
+    x = inputs.generate(w, "cuda")
+    out = [torch.empty((S, N), dtype=torch.float32 if k % 3 == 0 else torch.int32, device="cuda") for k in range(6)]
+    plan = hs.hs_plan(N, S, H)
+    try:
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+        hs.hs_plan_set_tuning(plan, 0)
+        hs.hs_run_greedy(plan, x, None, mu, sg, out[0], out[1], out[2])
+        assert hs.hs_last_kernel(plan).startswith("hs_greedy_tile_kernel")
+        hs.hs_plan_set_tuning(plan, GENERIC)
+        hs.hs_run_greedy(plan, x, None, mu, sg, out[3], out[4], out[5])
+        assert hs.hs_last_kernel(plan).startswith("hs_greedy_generic_kernel")
+        torch.cuda.synchronize()
+        assert torch.equal(out[2], out[5]) and torch.equal(out[1], out[4])
+        assert torch.equal(out[0].view(torch.int32), out[3].view(torch.int32))
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+        for content in ("cfg3", "integer"):
+            if content == "integer":
+                g = torch.Generator(device="cuda"); g.manual_seed(9)
+                for s in range(S):
+                    x[s] = torch.randint(0, 64, (N,), generator=g, device="cuda", dtype=torch.int32).to(torch.float32)
+                mu, sg = _int_stats(H)
+            hs.hs_plan_set_tuning(plan, 0)
+            hs.hs_run_presto(plan, x, None, mu, sg, out[0], out[1])
+            assert hs.hs_last_kernel(plan).startswith("hs_presto_rows_kernel")
+            hs.hs_plan_set_tuning(plan, GENERIC)
+            hs.hs_run_presto(plan, x, None, mu, sg, out[3], out[4])
+            assert hs.hs_last_kernel(plan).startswith("hs_presto_generic_kernel")
+            torch.cuda.synchronize()
+            if content == "integer":
+                assert torch.equal(out[1], out[4]) and torch.equal(out[0].view(torch.int32), out[3].view(torch.int32))
+                rng = np.random.default_rng(3)
+                rows = np.repeat(np.array([0, 100, S - 1]), 2000)
+                bins = np.tile(_sample_bins(N, rng, 900)[:2000], 3)
+                hrows = {r: x[r].cpu().numpy() for r in (0, 100, S - 1)}
+                for r in (0, 100, S - 1):
+                    bsel = bins[rows == r]
+                    ref = oracle_mod.presto_bins(hrows[r][None, :], H, mu, sg, np.zeros_like(bsel), bsel)
+                    idx = torch.from_numpy(bsel).cuda()
+                    assert np.array_equal(out[1][r, idx].cpu().numpy(), ref["best_h"])
+                    assert np.array_equal(out[0][r, idx].cpu().numpy().astype(np.float64), ref["snr"])
+            else:
+                err = (out[0] - out[3]).abs()
+                bound = 1e-5 * (out[3].abs() + float(mu[-1]) / float(sg[-1]) + 1.0)
+                assert bool((err <= bound).all())
+                mism = int((out[1] != out[4]).sum())
+                assert mism <= 1e-4 * S * N, mism          # near-ties only (their snr already agree within the bound)
+            del_err = None
+    finally:
+        hs.hs_destroy(plan)
+
+
+# ------------------------------------------------------------------------------------------
+# configs[3] at its real size: 1024 x 2^21 = 2^31 elements per array, row offsets beyond int32
+# ------------------------------------------------------------------------------------------
+def test_cfg4_full_size(hs, oracle_mod):
+    """One hs_run_greedy call over the whole cfg4 batch with its whitening multiplier (reading R13).  Rows 0, 511,
+    512 and 1023 (element offsets below, at and beyond 2^31) are compared with the oracle element by element
+    (path bit-exact), and every row of the tile kernel is compared bit for bit with the generic 64-bit kernel."""
+    from parity import check_greedy
+    w = inputs.workload("cfg4")
+    S, N, H = w.n_spectra, w.n_bins, w.H
+    assert S * N == 1 << 31
+    free, _ = torch.cuda.mem_get_info()
+    if free < 72 * (1 << 30):
+        pytest.skip("needs 72 GiB of device memory")
+    x = inputs.generate(w, "cuda")
+    ib = torch.empty_like(x)
+    for s0 in range(0, S, 64):
+        ib[s0:s0 + 64] = inputs.block_median_inv_baseline(x[s0:s0 + 64])
+    out = [torch.empty((S, N), dtype=torch.float32 if k % 3 == 0 else torch.int32, device="cuda") for k in range(6)]
+    mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", H))
+    plan = hs.hs_plan(N, S, H)
+    try:
+        hs.hs_run_greedy(plan, x, ib, mu, sg, out[0], out[1], out[2])
+        assert hs.hs_last_kernel(plan).startswith("hs_greedy_tile_kernel")
+        hs.hs_plan_set_tuning(plan, GENERIC)
+        hs.hs_run_greedy(plan, x, ib, mu, sg, out[3], out[4], out[5])
+        assert hs.hs_last_kernel(plan).startswith("hs_greedy_generic_kernel")
+        torch.cuda.synchronize()
+    finally:
+        hs.hs_destroy(plan)
+    assert torch.equal(out[2], out[5]) and torch.equal(out[1], out[4])
+    assert torch.equal(out[0].view(torch.int32), out[3].view(torch.int32))
+    rows = [0, 511, 512, S - 1]
+    check_greedy(oracle_mod, x[rows].cpu().numpy(), H, mu, sg, 0, out[0][rows].cpu().numpy(), out[1][rows].cpu().numpy(),
+                 out[2][rows].cpu().numpy(), inv_baseline=ib[rows].cpu().numpy(), T=10.0)
