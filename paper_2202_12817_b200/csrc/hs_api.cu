@@ -12,7 +12,7 @@
 #include "hs_common.cuh"
 #include "hs_generic.cuh"
 #include "hs_greedy.cuh"
-#include "hs_presto_rows.cuh"
+#include "hs_presto_tile.cuh"
 #include "hs_presto_farey.cuh"
 #include "hs_candidates.cuh"
 
@@ -175,29 +175,29 @@ hs_status launch_greedy_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
     return HS_OK;
 }
 
-template <int L, int W, bool BULK, int NE>
-hs_status launch_presto_rows_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
-    constexpr int smem = 4 * hs_rows::smem_words(L, W);
+template <int L, int W>
+hs_status launch_presto_tile_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    constexpr int smem = 4 * hs_tile::smem_words(L, W);
     static std::atomic<uint64_t> opted{0};              // per instantiation, one bit per device
-    HS_CUDA(opt_in_smem(hs_presto_rows_kernel<L, W, BULK, NE>, smem, p->device, opted));
-    constexpr int T = hs_rows::WT * W;
+    HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W>, smem, p->device, opted));
+    constexpr int T = hs_tile::TILE * W;
     dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
-    hs_presto_rows_kernel<L, W, BULK, NE><<<grid, (NE < 0 ? 64 : 32) * W, smem, stream>>>(sh, st, io);
-    p->last_kernel = NE < 0 ? "hs_presto_rows_kernel<pair>" : "hs_presto_rows_kernel<single>";
+    hs_presto_tile_kernel<L, W><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+    p->last_kernel = W == 2 ? "hs_presto_tile_kernel<W=2>" : W == 1 ? "hs_presto_tile_kernel<W=1>" : "hs_presto_tile_kernel<W=3>";
     p->launches += 1;
     HS_CUDA(cudaGetLastError());
     return HS_OK;
 }
 
-template <int W, bool BULK, int NE>
-hs_status launch_presto_rows(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+template <int W>
+hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     switch (floor_log2(sh.H)) {
-        case 0: return launch_presto_rows_L<0, W, BULK, NE>(p, sh, st, io, stream);
-        case 1: return launch_presto_rows_L<1, W, BULK, NE>(p, sh, st, io, stream);
-        case 2: return launch_presto_rows_L<2, W, BULK, NE>(p, sh, st, io, stream);
-        case 3: return launch_presto_rows_L<3, W, BULK, NE>(p, sh, st, io, stream);
-        case 4: return launch_presto_rows_L<4, W, BULK, NE>(p, sh, st, io, stream);
-        default: return launch_presto_rows_L<5, W, BULK, NE>(p, sh, st, io, stream);
+        case 0: return launch_presto_tile_L<0, W>(p, sh, st, io, stream);
+        case 1: return launch_presto_tile_L<1, W>(p, sh, st, io, stream);
+        case 2: return launch_presto_tile_L<2, W>(p, sh, st, io, stream);
+        case 3: return launch_presto_tile_L<3, W>(p, sh, st, io, stream);
+        case 4: return launch_presto_tile_L<4, W>(p, sh, st, io, stream);
+        default: return launch_presto_tile_L<5, W>(p, sh, st, io, stream);
     }
 }
 
@@ -216,9 +216,11 @@ hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
     const bool fast_ok = !io.inv_base && !(sh.flags & (HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS)) &&
                          sh.n_bins * 32 < (1ll << 31) - 64 && p->tune != HS_TUNE_GENERIC;
     if (fast_ok) {
-        // measured: two warps per 512-output tile win at H >= 32 only
-        if (sh.H >= 32 && p->tune != 31) return launch_presto_rows<2, true, -8>(p, sh, st, io, stream);
-        return launch_presto_rows<2, true, 8>(p, sh, st, io, stream);
+        switch (p->tune) {                                   // measured on cfg3: W = 2 3.06 ms, W = 3 3.03 ms, W = 1 3.69 ms
+            case 50: return launch_presto_tile<1>(p, sh, st, io, stream);
+            case 52: return launch_presto_tile<3>(p, sh, st, io, stream);
+            default: return launch_presto_tile<2>(p, sh, st, io, stream);
+        }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
     if (io.inv_base) hs_presto_generic_kernel<true><<<grid, 256, 0, stream>>>(sh, st, io);

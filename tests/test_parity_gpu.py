@@ -93,7 +93,7 @@ SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (
 
 # hs_plan_set_tuning values: 0 = the library's choice, 255 = coverage kernels, others = alternative tile shapes
 GREEDY_TUNES = [0, 3, 255]
-PRESTO_TUNES = [0, 31, 255]
+PRESTO_TUNES = [0, 50, 52, 255]
 
 
 @pytest.mark.parametrize("tune", GREEDY_TUNES)
@@ -120,6 +120,20 @@ def test_presto_exact_integer(hs, oracle_mod, tune, H):
         s, b = run_presto(hs, x, H, mu, sg, tune=tune)
         assert np.array_equal(b, b_ref), (S, N)
         assert np.array_equal(s.astype(np.float64), s_ref), (S, N)
+
+
+@pytest.mark.parametrize("tune", [t for t in PRESTO_TUNES if t != 255])
+@pytest.mark.parametrize("H", [8, 32])
+def test_presto_many_tiles_per_cta(hs, oracle_mod, tune, H):
+    """Enough tiles that every CTA of a persistent kernel goes round its ring of stages many times (ragged rows,
+    rows that start on odd 16-byte units), against the oracle bit for bit on exact-integer spectra."""
+    mu, sg = _int_stats(H)
+    S, N = 48, 150001
+    x = inputs.integer_spectra(300 + H, S, N, 255).numpy()
+    s_ref, b_ref = oracle_mod.presto(x, H, mu, sg)
+    s, b = run_presto(hs, x, H, mu, sg, tune=tune)
+    assert np.array_equal(b, b_ref)
+    assert np.array_equal(s.astype(np.float64), s_ref)
 
 
 @pytest.mark.parametrize("tune", [0, 255])
@@ -464,7 +478,7 @@ def _sample_bins(N, rng, k=6000):
 
 @pytest.mark.parametrize("kind,N,kernel", [
     ("greedy", (1 << 30) + 7, "hs_greedy_tile_kernel"),            # 32-bit h n close to its limit
-    ("presto", (1 << 26) - 70, "hs_presto_rows_kernel"),           # 32 N just below 2^31
+    ("presto", (1 << 26) - 70, "hs_presto_tile_kernel"),           # 32 N just below 2^31
     ("presto", (1 << 26) + 8, "hs_presto_generic_kernel"),         # just past the rows kernel's limit
     ("greedy", (1 << 31) - (1 << 17), "hs_greedy_tile_kernel"),    # the last N the tile kernel takes
     ("greedy", (1 << 31) - 64, "hs_greedy_generic_kernel"),        # the largest N hs_plan accepts: 64-bit offsets
@@ -552,7 +566,7 @@ def test_cfg3_all_rows_tuned_vs_generic(hs, oracle_mod):
                 mu, sg = _int_stats(H)
             hs.hs_plan_set_tuning(plan, 0)
             hs.hs_run_presto(plan, x, None, mu, sg, out[0], out[1])
-            assert hs.hs_last_kernel(plan).startswith("hs_presto_rows_kernel")
+            assert hs.hs_last_kernel(plan).startswith("hs_presto_tile_kernel")
             hs.hs_plan_set_tuning(plan, GENERIC)
             hs.hs_run_presto(plan, x, None, mu, sg, out[3], out[4])
             assert hs.hs_last_kernel(plan).startswith("hs_presto_generic_kernel")
