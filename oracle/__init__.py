@@ -56,6 +56,8 @@ def _load():
                                               c_d, c_i32, c_u32, c_d, c_i64]
         lib.hs_oracle_presto_bins.argtypes = [c_f, c_f, i64, i64, i32, c_f, c_f, u32, c_i64, c_i64, i64,
                                               c_d, c_i32, c_d]
+        lib.hs_oracle_estimate_stats.argtypes = [c_f, c_f, i64, i32, i64, i32, u32, i32, i64, i64,
+                                                 ctypes.c_double, i32, c_f, c_f, c_i64]
         lib.hs_oracle_presto_index.argtypes = [i32, i32, i64]
         lib.hs_oracle_presto_index.restype = i64
         lib.hs_oracle_presto_order_in_set.argtypes = [i32, u32]
@@ -186,6 +188,25 @@ def presto_bins(x, H: int, mu, sigma, rows, bins, flags: int = 0, inv_baseline=N
     if rc != 0:
         raise ValueError("hs_oracle_presto_bins: invalid arguments")
     return dict(snr=snr, best_h=bh, snr_h=snr_h)
+
+
+def estimate_stats(x, H: int, flags: int = 0, greedy: bool = True, n_lo: int = 0, n_hi: Optional[int] = None,
+                   clip: float = 3.0, n_clip: int = 0, inv_baseline=None):
+    """Reading R14 of GetMeanStdev(): per spectrum and order h, mean and standard deviation
+    over n in [n_lo, n_hi) of the variant's partial sum S_h(n), with n_clip rounds of outlier rejection at
+    mean +/- clip * std.  Returns (mu [S,H] float32, sigma [S,H] float32, count [S,H] int64)."""
+    lib = _load()
+    a = _as_f32_2d(x)
+    S, N = a.shape
+    ib = None if inv_baseline is None else _as_f32_2d(inv_baseline)
+    n_hi = N if n_hi is None else n_hi
+    mu = np.empty((S, H), np.float32); sg = np.empty((S, H), np.float32); cnt = np.empty((S, H), np.int64)
+    rc = lib.hs_oracle_estimate_stats(_ptr(a, ctypes.c_float), _ptr(ib, ctypes.c_float), N, S, N, H, flags,
+                                      1 if greedy else 0, n_lo, n_hi, float(clip), n_clip,
+                                      _ptr(mu, ctypes.c_float), _ptr(sg, ctypes.c_float), _ptr(cnt, ctypes.c_int64))
+    if rc != 0:
+        raise ValueError("hs_oracle_estimate_stats: invalid arguments")
+    return mu, sg, cnt
 
 
 def presto_index(h: int, Hp: int, n: int) -> int:

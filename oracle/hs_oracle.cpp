@@ -34,6 +34,14 @@
 //       so best_h is in [1, H].                                                 [parity unpinned]
 //   R7  fundamental selection on by default; a flag disables it.
 //   R8  mu[h-1], sigma[h-1] are inputs (the statistics of the partial sum at order h).
+//   R14 GetMeanStdev() ("mean and standard deviation for partial sum of length H", PAPER.md:58;
+//       "all algorithms use the same pre-processing steps (mean and standard deviation calculation ...)")
+//       is not defined by the paper.  Reading (hs_oracle_estimate_stats below): per spectrum and per order h, the
+//       sample mean and the population standard deviation, over the bins n of a caller-chosen range [n_lo, n_hi), of
+//       the partial sum S_h(n) that the selected variant forms at order h (bins whose order h is not evaluated do not
+//       count), followed by n_clip rounds of outlier rejection: round p keeps the sums with
+//       lo <= S_h(n) <= hi, lo/hi = mean -/+ clip * std of round p-1 rounded to fp32.  An order without samples gets
+//       (mu, sigma) = (0, 1); a zero standard deviation is returned as 1.
 //   NEXT-2: an optional per-bin multiplier inv_baseline[] whitens the spectrum; the product
 //       x*inv_baseline is formed in fp32 (one IEEE multiply -- the kernel's precision --
 //       because it decides the greedy comparison), everything after it in fp64.
@@ -45,6 +53,7 @@
 // Parity unpinned by anything the paper prints: R3 (tie rule of Round), R4 (band edge),
 // R6 (tie-breaks); they are fixed by the readings above.
 // =====================================================================================
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -255,6 +264,54 @@ int hs_oracle_presto_bins(const float* x, const float* inv_baseline, int64_t N, 
         if (bins[i] < 0 || bins[i] >= N) return 1;
         const Spectrum sp{x + rows[i] * in_stride, inv_baseline ? inv_baseline + rows[i] * in_stride : nullptr, N};
         presto_bin(sp, H, st, flags, bins[i], &snr[i], &best_h[i], snr_h ? snr_h + i * H : nullptr);
+    }
+    return 0;
+}
+
+// R14: the statistics of the partial sums (the reading of GetMeanStdev() in the header).  greedy != 0: Alg. 2 with
+// `flags`; else the PRESTO family with `flags` (orders outside its order set get (0, 1)).
+// mu, sigma: [S][H] fp32 out; count: [S][H] int64 out (samples kept in the last round; nullable).
+int hs_oracle_estimate_stats(const float* x, const float* inv_baseline, int64_t N, int32_t S, int64_t in_stride,
+                             int32_t H, uint32_t flags, int32_t greedy, int64_t n_lo, int64_t n_hi,
+                             double clip, int32_t n_clip, float* mu, float* sigma, int64_t* count) {
+    if (!x || !mu || !sigma || N < 2 || S < 1 || H < 1 || H > 32 || in_stride < N) return 1;
+    if (n_lo < 0 || n_hi > N || n_lo > n_hi || n_clip < 0 || !(clip > 0.0)) return 1;
+    if (!greedy && (flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    std::vector<float> zero(H, 0.0f), one(H, 1.0f);
+    const Stats unit{zero.data(), one.data()};               // (sum - 0) / 1 = the partial sum itself
+    std::vector<double> sums(H);
+    for (int32_t s = 0; s < S; ++s) {
+        const Spectrum sp{x + (int64_t)s * in_stride, inv_baseline ? inv_baseline + (int64_t)s * in_stride : nullptr, N};
+        std::vector<double> lo(H, NEG_INF), hi(H, -NEG_INF), mean(H, 0.0), sd(H, 0.0);
+        std::vector<int64_t> cnt(H, 0);
+        for (int p = 0; p <= n_clip; ++p) {
+            std::vector<double> a1(H, 0.0), a2(H, 0.0);
+            std::fill(cnt.begin(), cnt.end(), 0);
+            for (int64_t n = n_lo; n < n_hi; ++n) {
+                double best; int32_t bh;
+                if (greedy) greedy_bin(sp, H, unit, flags, n, &best, &bh, nullptr, sums.data(), nullptr);
+                else presto_bin(sp, H, unit, flags, n, &best, &bh, sums.data());
+                for (int h = 0; h < H; ++h) {
+                    const double v = sums[h];
+                    if (v != v) continue;                    // order not evaluated for this bin
+                    if (v < lo[h] || v > hi[h]) continue;    // rejected by the previous round
+                    cnt[h] += 1; a1[h] += v; a2[h] += v * v;
+                }
+            }
+            for (int h = 0; h < H; ++h) {
+                if (cnt[h] == 0) { mean[h] = 0.0; sd[h] = 0.0; continue; }
+                mean[h] = a1[h] / (double)cnt[h];
+                const double var = a2[h] / (double)cnt[h] - mean[h] * mean[h];
+                sd[h] = var > 0.0 ? std::sqrt(var) : 0.0;
+                lo[h] = (double)(float)(mean[h] - clip * sd[h]);
+                hi[h] = (double)(float)(mean[h] + clip * sd[h]);
+            }
+        }
+        for (int h = 0; h < H; ++h) {
+            mu[(int64_t)s * H + h] = cnt[h] ? (float)mean[h] : 0.0f;
+            sigma[(int64_t)s * H + h] = (cnt[h] && sd[h] > 0.0) ? (float)sd[h] : 1.0f;
+            if (count) count[(int64_t)s * H + h] = cnt[h];
+        }
     }
     return 0;
 }

@@ -512,3 +512,90 @@ def test_candidates_definition_brute_force():
     got, vals = oracle.candidates(snr, bh, 10.0)
     assert [tuple(r) for r in got.tolist()] == want == [(0, 1, 2), (0, 3, 4), (1, 1, 6), (1, 3, 8)]
     assert vals.tolist() == [float(snr[s, n]) for s, n, _ in want]
+
+
+# ------------------------------------------------------------------------------------------
+# R14: the reading of GetMeanStdev() -- oracle.estimate_stats
+# ------------------------------------------------------------------------------------------
+def _simple_sums_numpy(x, H, n_lo, n_hi):
+    """S_h(n) = sum_{k<=h} x[k n] (eq. 3) by gather + cumsum; NaN where h n > N - 1.  Independent of the oracle."""
+    N = x.shape[0]
+    n = np.arange(n_lo, n_hi)
+    out = np.full((n.size, H), np.nan)
+    run = np.zeros(n.size)
+    alive = np.ones(n.size, bool)
+    for h in range(1, H + 1):
+        alive &= h * n <= N - 1
+        run[alive] += x[(h * n)[alive]].astype(np.float64)
+        out[alive, h - 1] = run[alive]
+    return out
+
+
+def test_r14_stats_simple_variant_equals_numpy_moments(oracle_mod):
+    """Exact-integer spectra, simple harmonic sum: mean / population std / count of S_h over a range that crosses the
+    band edges N/h, against numpy moments of numpy gathers (nothing of the oracle is re-used)."""
+    H, N = 16, 6000
+    x = inputs.integer_spectra(71, 3, N, 50).numpy()
+    n_lo, n_hi = 5, 2500
+    mu, sg, cnt = oracle_mod.estimate_stats(x, H, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi)
+    for s in range(3):
+        sums = _simple_sums_numpy(x[s], H, n_lo, n_hi)
+        for h in range(H):
+            v = sums[:, h][~np.isnan(sums[:, h])]
+            assert cnt[s, h] == v.size == np.count_nonzero((h + 1) * np.arange(n_lo, n_hi) <= N - 1)
+            assert mu[s, h] == np.float32(v.mean())
+            assert abs(float(sg[s, h]) - v.std()) <= 1e-6 * v.std()
+
+
+def test_r14_stats_clipping_rounds(oracle_mod):
+    """Outlier rejection: a few enormous bins; each round keeps the sums inside mean -/+ clip std of the round before
+    (fp32-rounded limits).  Re-done in numpy for the simple variant."""
+    H, N, clip = 8, 40000, 2.5
+    x = inputs.integer_spectra(72, 1, N, 20).numpy()
+    x[0, ::997] += 5000.0
+    n_lo, n_hi = 100, 4000
+    sums = _simple_sums_numpy(x[0], H, n_lo, n_hi)
+    for n_clip in (0, 1, 3):
+        mu, sg, cnt = oracle_mod.estimate_stats(x, H, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, clip=clip, n_clip=n_clip)
+        for h in range(H):
+            v = sums[:, h]
+            keep = np.ones(v.size, bool)
+            for _ in range(n_clip + 1):
+                m, sd = v[keep].mean(), v[keep].std()
+                stats = (m, sd, int(keep.sum()))
+                lo, hi = np.float32(m - clip * sd), np.float32(m + clip * sd)
+                keep = (v >= lo) & (v <= hi)
+            assert cnt[0, h] == stats[2]
+            assert mu[0, h] == np.float32(stats[0]) and abs(float(sg[0, h]) - stats[1]) <= 1e-6 * stats[1]
+        if n_clip:
+            assert cnt[0, 0] < n_hi - n_lo and mu[0, 0] < 15.0          # the outliers are gone: mean of U{0..20} = 10
+
+
+def test_r14_stats_closed_forms_and_degenerate_cases(oracle_mod):
+    """Exp(1) noise: greedy mean 1.5 h, variance 1.25 h; PRESTO (Alg. 1) t terms; PRESTO_all H' terms (SURVEY.md 8(c)
+    statistics paragraph) within sampling error.  Constant spectrum: mean h c, sigma returned as 1.  Orders outside
+    the PRESTO order set: (0, 1) with no samples."""
+    H = 16
+    x = inputs.generate(inputs.Workload("n", 2, 1 << 19, H, seed=91)).numpy()
+    n_lo, n_hi = 2000, 30000
+    k = n_hi - n_lo
+    mu, sg, cnt = oracle_mod.estimate_stats(x, H, 0, True, n_lo, n_hi)
+    h = np.arange(1, H + 1)
+    assert np.all(cnt == k)
+    # neighbouring n share bins, so the sums are correlated: bounds in relative terms, not in iid standard errors
+    assert np.all(np.abs(mu / (1.5 * h) - 1.0) <= 0.02)
+    assert np.all(np.abs(sg ** 2 / (1.25 * h) - 1.0) <= 0.08)
+    mu, sg, cnt = oracle_mod.estimate_stats(x, H, 0, False, n_lo, n_hi)
+    for Hp in range(1, H + 1):
+        if Hp & (Hp - 1):
+            assert np.all(cnt[:, Hp - 1] == 0) and np.all(mu[:, Hp - 1] == 0.0) and np.all(sg[:, Hp - 1] == 1.0)
+        else:
+            t = 1.0 if Hp == 1 else 1.0 + Hp // 2
+            assert np.all(np.abs(mu[:, Hp - 1] / t - 1.0) <= 0.03)
+            assert np.all(np.abs(sg[:, Hp - 1] ** 2 / t - 1.0) <= 0.12)
+    mu, sg, cnt = oracle_mod.estimate_stats(x, H, ALL_HARMONICS, False, n_lo, n_hi)
+    for Hp in (1, 2, 4, 8, 16):
+        assert np.all(np.abs(mu[:, Hp - 1] / Hp - 1.0) <= 0.03)
+    c = np.full((1, 5000), 3.0, np.float32)
+    mu, sg, cnt = oracle_mod.estimate_stats(c, 8, 0, True, 10, 500)
+    assert np.array_equal(mu[0], 3.0 * np.arange(1, 9)) and np.all(sg == 1.0)
