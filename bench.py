@@ -65,6 +65,9 @@ def parse_args():
                     help="which forms a step runs (cfg4 is quoted on the greedy form only)")
     ap.add_argument("--greedy-flags", type=int, default=0, help="HS_GREEDY_* plan flags (NEXT-1 variants)")
     ap.add_argument("--presto-flags", type=int, default=0, help="HS_PRESTO_* plan flags (NEXT-1 variants)")
+    ap.add_argument("--stats", default="auto", choices=["auto", "given", "estimated"],
+                    help="given: closed-form Exp(1) statistics passed by value; estimated: hs_estimate_stats (reading R14 of "
+                         "GetMeanStdev) inside the step, then hs_run_*_dstats; auto = estimated for the red-noise workload (cfg4)")
     ap.add_argument("--tune-greedy", type=int, default=0)
     ap.add_argument("--tune-presto", type=int, default=0)
     return ap.parse_args()
@@ -267,22 +270,43 @@ def run_cuda(args):
     hs.hs_plan_set_tuning(plan_g, args.tune_greedy)     # 0 = the library's choice (diagnostic knob)
     hs.hs_plan_set_tuning(plan_p, args.tune_presto)
     stream = torch.cuda.current_stream(dev)
+    # NEXT-2: the statistics estimated on the device inside the step (two rejection rounds at 3 sigma over the
+    # fundamentals / top bins [N/64, N/32), where every order exists), then per-spectrum statistics from device memory
+    est = args.stats == "estimated" or (args.stats == "auto" and w.red_noise)
+    n_clip, clip = 2, 3.0
+    if est:
+        dmu_g = torch.empty((S, H), dtype=torch.float32, device=dev); dsg_g = torch.empty_like(dmu_g)
+        dmu_p = torch.empty_like(dmu_g); dsg_p = torch.empty_like(dmu_g)
+        work = torch.empty(hs.hs_stats_workspace_bytes(plan_g, n_clip) // 8, dtype=torch.float64, device=dev)
 
     def step(ev=None):
         if ev is not None:
             ev[0].record(stream)
+        if est:
+            if do_g:
+                hs.hs_estimate_stats(plan_g, True, x, ib, N // 64, N // 32, clip, n_clip, dmu_g, dsg_g, work, stream.cuda_stream)
+            if do_p:
+                hs.hs_estimate_stats(plan_p, False, x, ib, N // 64, N // 32, clip, n_clip, dmu_p, dsg_p, work, stream.cuda_stream)
+        if ev is not None:
+            ev[3].record(stream)
         if do_g:
-            hs.hs_run_greedy(plan_g, x, ib, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
+            if est:
+                hs.hs_run_greedy_dstats(plan_g, x, ib, dmu_g, dsg_g, snr_g, bh_g, None, stream.cuda_stream)
+            else:
+                hs.hs_run_greedy(plan_g, x, ib, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
         if ev is not None:
             ev[1].record(stream)
         if do_p:
-            hs.hs_run_presto(plan_p, x, ib, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
+            if est:
+                hs.hs_run_presto_dstats(plan_p, x, ib, dmu_p, dsg_p, snr_p, bh_p, stream.cuda_stream)
+            else:
+                hs.hs_run_presto(plan_p, x, ib, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
         if ev is not None:
             ev[2].record(stream)
 
     for _ in range(args.warmup):
         step()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -295,7 +319,8 @@ def run_cuda(args):
     launches = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p) - l0
     kname = {"greedy": hs.hs_last_kernel(plan_g) if do_g else None, "presto": hs.hs_last_kernel(plan_p) if do_p else None}
     total_ms = evs[0][0].elapsed_time(evs[-1][2])          # device time of exactly K steps
-    g_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    s_ms = sum(e[0].elapsed_time(e[3]) for e in evs) / args.steps
+    g_ms = sum(e[3].elapsed_time(e[1]) for e in evs) / args.steps
     p_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
     # clocks: keep the sampler running through a few more device-only steps so short runs still get samples
     if rank == 0:
@@ -309,6 +334,7 @@ def run_cuda(args):
     total_ms = max_over_ranks(total_ms, dev)
     g_ms = max_over_ranks(g_ms, dev)
     p_ms = max_over_ranks(p_ms, dev)
+    s_ms = max_over_ranks(s_ms, dev)
     bins_step = float(S) * N * world
     n_forms = int(do_g) + int(do_p)
     default_run = (args.forms == "both" and not args.greedy_flags and not args.presto_flags and ib is None
@@ -441,6 +467,9 @@ def run_cuda(args):
                                        (", per-bin inverse baseline" if ib is not None else ""),
                            "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
+                "stats": ({"source": "hs_estimate_stats inside the step (reading R14): bins [N/64, N/32), 2 rejection rounds at 3 sigma, "
+                                     "then hs_run_*_dstats", "ms": s_ms} if est else
+                          {"source": "closed-form Exp(1) statistics passed by value", "ms": 0.0}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "candidates": cand,
                 "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)

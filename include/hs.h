@@ -20,7 +20,7 @@
  *   N = n_bins per spectrum, S = n_spectra, x[s][b] the power of spectrum s at bin b,
  *   H = maximum harmonic order (1..32).  mu[h-1], sigma[h-1] are the mean and standard
  *   deviation of the partial sum at harmonic order h; the library never
- *   estimates them ("GetMeanStdev()", is the caller's).
+ *   estimates them inside hs_run_* ("GetMeanStdev()", is a step of its own: hs_estimate_stats).
  *   Outputs are written for every bin n in [0, n_fund) of every spectrum; for the greedy
  *   form n is the FUNDAMENTAL bin, for the PRESTO form n is the TOP (last-summed) bin
  *   (PAPER.md:140).
@@ -127,6 +127,37 @@ hs_status hs_run_greedy(hs_plan_t plan, const float* d_spectra, const float* d_i
 hs_status hs_run_presto(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
                         const float* mu, const float* sigma,
                         float* d_snr, int32_t* d_best_h, void* cuda_stream);
+
+/* The same two operations with PER-SPECTRUM statistics that already live on the device (the output of
+ * hs_estimate_stats, or the caller's own): d_mu, d_sigma are DEVICE arrays [S][H] of fp32, entry [s][h-1] for order h
+ * of spectrum s; every CTA forms 1/sigma and -mu/sigma of its spectrum exactly as the host does for the by-value
+ * statistics.  sigma must be > 0 (not checked: the values are never read on the host).  Otherwise as hs_run_greedy /
+ * hs_run_presto: asynchronous, no allocation, no synchronisation. */
+hs_status hs_run_greedy_dstats(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
+                               const float* d_mu, const float* d_sigma,
+                               float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream);
+hs_status hs_run_presto_dstats(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
+                               const float* d_mu, const float* d_sigma,
+                               float* d_snr, int32_t* d_best_h, void* cuda_stream);
+
+/* The step before the path: "{mu, sigma} = GetMeanStdev()", "the mean and standard deviation ...
+ * for partial sum of length H", the pre-processing all algorithms share.  The paper does
+ * not define it; reading R14 of DESIGN.md: for every spectrum s and order h, the mean and the population standard
+ * deviation over the bins n in [n_lo, n_hi) of the partial sum S_h(n) that the selected form builds at order h
+ * (greedy != 0: Alg. 2 with the plan's greedy flags, n the fundamental bin, bins whose order h lies beyond the band
+ * edge do not count; greedy == 0: the Alg. 1 family with the plan's PRESTO flags, n the top bin, H' outside the order
+ * set get (0, 1)), with the whitening multiplier applied if d_inv_baseline != NULL, followed by n_clip rounds of
+ * outlier rejection: round p keeps the sums with lo <= S_h(n) <= hi, lo / hi = mean -/+ clip_sigma * std of round
+ * p - 1 rounded to fp32.  An order without samples gets (0, 1); a zero deviation is returned as 1.
+ *   n_lo, n_hi   bin range (n_hi = 0: n_bins)
+ *   d_mu, d_sigma  [S][H] fp32 out (device): the arguments hs_run_*_dstats take
+ *   d_work       device workspace of hs_stats_workspace_bytes(plan, n_clip) bytes, 8-byte aligned (zeroed by the call)
+ * S_h is accumulated in fp32 as the coverage kernels do; the moments in fp64 (the order of the fp64 additions is not
+ * fixed).  Asynchronous on the stream: n_clip + 1 gather passes over [n_lo, n_hi) and one tiny launch. */
+hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
+                            int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
+                            float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream);
+int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip);   /* -1 on invalid arguments (n_clip in 0..16) */
 
 /* The same two operations with HOST buffers (any host memory; page-locked memory copies
  * fastest).  Spectra are streamed through plan-owned device staging buffers in groups of

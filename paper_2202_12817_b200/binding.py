@@ -26,6 +26,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
+           "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -68,6 +69,14 @@ def load() -> ctypes.CDLL:
     lib.hs_plan_set_tuning.restype = ctypes.c_int
     lib.hs_find_candidates.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp, vp]
     lib.hs_find_candidates.restype = ctypes.c_int
+    lib.hs_run_greedy_dstats.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.hs_run_greedy_dstats.restype = ctypes.c_int
+    lib.hs_run_presto_dstats.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.hs_run_presto_dstats.restype = ctypes.c_int
+    lib.hs_estimate_stats.argtypes = [vp, i32, vp, vp, i64, i64, ctypes.c_float, i32, vp, vp, vp, i64, vp]
+    lib.hs_estimate_stats.restype = ctypes.c_int
+    lib.hs_stats_workspace_bytes.argtypes = [vp, i32]
+    lib.hs_stats_workspace_bytes.restype = i64
     lib.hs_launch_count.argtypes = [vp]
     lib.hs_launch_count.restype = i64
     lib.hs_last_kernel.argtypes = [vp]
@@ -140,6 +149,50 @@ def hs_run_presto(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.
                              _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), _farr(mu), _farr(sigma),
                              _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
                              stream), "hs_run_presto")
+
+
+def hs_run_greedy_dstats(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor], d_mu: torch.Tensor,
+                         d_sigma: torch.Tensor, d_snr: torch.Tensor, d_best_h: torch.Tensor,
+                         d_path: Optional[torch.Tensor] = None, stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_run_greedy_dstats(plan, _dptr(d_spectra, torch.float32, "d_spectra"),
+                                    _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"),
+                                    _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"),
+                                    _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                                    _dptr(d_path, torch.int32, "d_path"), stream), "hs_run_greedy_dstats")
+
+
+def hs_run_presto_dstats(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor], d_mu: torch.Tensor,
+                         d_sigma: torch.Tensor, d_snr: torch.Tensor, d_best_h: torch.Tensor,
+                         stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_run_presto_dstats(plan, _dptr(d_spectra, torch.float32, "d_spectra"),
+                                    _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"),
+                                    _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"),
+                                    _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                                    stream), "hs_run_presto_dstats")
+
+
+def hs_stats_workspace_bytes(plan, n_clip: int) -> int:
+    return int(load().hs_stats_workspace_bytes(plan, n_clip))
+
+
+def hs_estimate_stats(plan, greedy: bool, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor],
+                      n_lo: int, n_hi: int, clip_sigma: float, n_clip: int, d_mu: torch.Tensor, d_sigma: torch.Tensor,
+                      d_work: torch.Tensor, stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    if not d_work.is_cuda or not d_work.is_contiguous():
+        raise TypeError("d_work: expected a contiguous CUDA tensor")
+    _check(lib.hs_estimate_stats(plan, 1 if greedy else 0, _dptr(d_spectra, torch.float32, "d_spectra"),
+                                 _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), n_lo, n_hi, clip_sigma, n_clip,
+                                 _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"),
+                                 d_work.data_ptr(), d_work.numel() * d_work.element_size(), stream), "hs_estimate_stats")
 
 
 def hs_run_greedy_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best_h, h_path=None) -> None:

@@ -15,6 +15,7 @@
 #include "hs_presto_tile.cuh"
 #include "hs_presto_farey.cuh"
 #include "hs_candidates.cuh"
+#include "hs_stats.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -99,6 +100,7 @@ HsIO io_at(const HsIO& io, const HsShape& sh, long long s0) {
     r.snr += s0 * sh.out_stride;
     r.best_h += s0 * sh.out_stride;
     if (r.path) r.path += s0 * sh.out_stride;
+    if (r.d_mu) { r.d_mu += s0 * sh.H; r.d_sigma += s0 * sh.H; }
     return r;
 }
 
@@ -120,6 +122,14 @@ int floor_log2(int v) { int l = 0; while ((2 << l) <= v) ++l; return l; }
 // ------------------------------------------------------------------------------------------
 // kernel selection + launch (device buffers).  `sh` may describe a sub-batch (host staging).
 // ------------------------------------------------------------------------------------------
+template <int BLOCK, int R, bool MIX, bool IB, bool DS>
+void launch_greedy_tile_k(bool fs, bool wp, dim3 grid, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true, IB, true, MIX, DS><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else if (fs) hs_greedy_tile_kernel<BLOCK, R, true, false, IB, true, MIX, DS><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else if (wp) hs_greedy_tile_kernel<BLOCK, R, false, true, IB, true, MIX, DS><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else hs_greedy_tile_kernel<BLOCK, R, false, false, IB, true, MIX, DS><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+}
+
 template <int BLOCK, int R, bool MIX>
 hs_status launch_greedy_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     const long long tile = (long long)BLOCK * R;
@@ -127,15 +137,10 @@ hs_status launch_greedy_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
     dim3 grid((unsigned)(MIX ? hs_greedy::mixed_grid(nt) : nt), (unsigned)sh.n_spectra);
     const bool fs = !(sh.flags & HS_GREEDY_NO_FUND_SELECT);
     const bool wp = io.path != nullptr;
-    if (io.inv_base) {
-        if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true, true, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-        else if (fs && !wp) hs_greedy_tile_kernel<BLOCK, R, true, false, true, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-        else if (!fs && wp) hs_greedy_tile_kernel<BLOCK, R, false, true, true, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-        else hs_greedy_tile_kernel<BLOCK, R, false, false, true, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-    } else if (fs && wp) hs_greedy_tile_kernel<BLOCK, R, true, true, false, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-    else if (fs && !wp) hs_greedy_tile_kernel<BLOCK, R, true, false, false, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-    else if (!fs && wp) hs_greedy_tile_kernel<BLOCK, R, false, true, false, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
-    else hs_greedy_tile_kernel<BLOCK, R, false, false, false, true, MIX><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    if (io.inv_base && io.d_mu) launch_greedy_tile_k<BLOCK, R, MIX, true, true>(fs, wp, grid, sh, st, io, stream);
+    else if (io.inv_base) launch_greedy_tile_k<BLOCK, R, MIX, true, false>(fs, wp, grid, sh, st, io, stream);
+    else if (io.d_mu) launch_greedy_tile_k<BLOCK, R, MIX, false, true>(fs, wp, grid, sh, st, io, stream);
+    else launch_greedy_tile_k<BLOCK, R, MIX, false, false>(fs, wp, grid, sh, st, io, stream);
     p->last_kernel = BLOCK == 128 ? (MIX ? "hs_greedy_tile_kernel<128,4,mix>" : "hs_greedy_tile_kernel<128,4>") : "hs_greedy_tile_kernel<256,4,mix>";
     p->launches += 1;
     HS_CUDA(cudaGetLastError());
@@ -145,7 +150,7 @@ hs_status launch_greedy_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
 hs_status launch_greedy_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     const bool no_drift = sh.flags & HS_GREEDY_NO_DRIFT;
     // the tile kernel keeps h n in 32 bits: h n < N + 32 * (tile of 1024 fundamentals)
-    const bool fast_ok = sh.n_bins <= (1ll << 31) - (1ll << 17) && p->tune != HS_TUNE_GENERIC && (!no_drift || !io.inv_base);
+    const bool fast_ok = sh.n_bins <= (1ll << 31) - (1ll << 17) && p->tune != HS_TUNE_GENERIC && (!no_drift || (!io.inv_base && !io.d_mu));
     if (fast_ok && no_drift) {                              // simple harmonic sum: the tile kernel without the second bin
         const long long tile = 128 * 4;
         dim3 grid((unsigned)hs_greedy::mixed_grid((int)((sh.n_fund + tile - 1) / tile)), (unsigned)sh.n_spectra);
@@ -160,14 +165,16 @@ hs_status launch_greedy_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
         return HS_OK;
     }
     if (fast_ok) {
-        switch (p->tune) {
+        switch (io.d_mu ? 0u : p->tune) {
             case 3: return launch_greedy_tile<256, 4, true>(p, sh, st, io, stream);
             case 4: return launch_greedy_tile<128, 4, false>(p, sh, st, io, stream);     // tiles in ascending order (no band mix)
             default: return launch_greedy_tile<128, 4, true>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
-    if (io.inv_base) hs_greedy_generic_kernel<true><<<grid, 256, 0, stream>>>(sh, st, io);
+    if (io.inv_base && io.d_mu) hs_greedy_generic_kernel<true, true><<<grid, 256, 0, stream>>>(sh, st, io);
+    else if (io.inv_base) hs_greedy_generic_kernel<true><<<grid, 256, 0, stream>>>(sh, st, io);
+    else if (io.d_mu) hs_greedy_generic_kernel<false, true><<<grid, 256, 0, stream>>>(sh, st, io);
     else hs_greedy_generic_kernel<false><<<grid, 256, 0, stream>>>(sh, st, io);
     p->last_kernel = "hs_greedy_generic_kernel";
     p->launches += 1;
@@ -179,10 +186,16 @@ template <int L, int W>
 hs_status launch_presto_tile_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     constexpr int smem = 4 * hs_tile::smem_words(L, W);
     static std::atomic<uint64_t> opted{0};              // per instantiation, one bit per device
-    HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W>, smem, p->device, opted));
+    static std::atomic<uint64_t> opted_ds{0};
     constexpr int T = hs_tile::TILE * W;
     dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
-    hs_presto_tile_kernel<L, W><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+    if (io.d_mu) {
+        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, true>, smem, p->device, opted_ds));
+        hs_presto_tile_kernel<L, W, true><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+    } else {
+        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, false>, smem, p->device, opted));
+        hs_presto_tile_kernel<L, W, false><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+    }
     p->last_kernel = W == 2 ? "hs_presto_tile_kernel<W=2>" : W == 1 ? "hs_presto_tile_kernel<W=1>" : "hs_presto_tile_kernel<W=3>";
     p->launches += 1;
     HS_CUDA(cudaGetLastError());
@@ -203,7 +216,7 @@ hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
 
 hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     // PRESTO_all, and PRESTO+ at H > 16 (measured: below that the coverage kernel is faster): hs_presto_farey.cuh
-    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && p->tune != HS_TUNE_GENERIC &&
+    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && !io.d_mu && p->tune != HS_TUNE_GENERIC &&
         (!(sh.flags & HS_PRESTO_ALL_ORDERS) || sh.H > 16 || p->tune == 1)) {
         dim3 fgrid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
         if (sh.flags & HS_PRESTO_ALL_ORDERS) hs_presto_farey_kernel<true><<<fgrid, 256, 0, stream>>>(sh, st, io);
@@ -216,14 +229,16 @@ hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
     const bool fast_ok = !io.inv_base && !(sh.flags & (HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS)) &&
                          sh.n_bins * 32 < (1ll << 31) - 64 && p->tune != HS_TUNE_GENERIC;
     if (fast_ok) {
-        switch (p->tune) {                                   // measured on cfg3: W = 2 3.06 ms, W = 3 3.03 ms, W = 1 3.69 ms
+        switch (io.d_mu ? 0u : p->tune) {                    // measured on cfg3: W = 2 3.06 ms, W = 3 3.03 ms, W = 1 3.69 ms
             case 50: return launch_presto_tile<1>(p, sh, st, io, stream);
             case 52: return launch_presto_tile<3>(p, sh, st, io, stream);
             default: return launch_presto_tile<2>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
-    if (io.inv_base) hs_presto_generic_kernel<true><<<grid, 256, 0, stream>>>(sh, st, io);
+    if (io.inv_base && io.d_mu) hs_presto_generic_kernel<true, true><<<grid, 256, 0, stream>>>(sh, st, io);
+    else if (io.inv_base) hs_presto_generic_kernel<true><<<grid, 256, 0, stream>>>(sh, st, io);
+    else if (io.d_mu) hs_presto_generic_kernel<false, true><<<grid, 256, 0, stream>>>(sh, st, io);
     else hs_presto_generic_kernel<false><<<grid, 256, 0, stream>>>(sh, st, io);
     p->last_kernel = "hs_presto_generic_kernel";
     p->launches += 1;
@@ -450,6 +465,84 @@ hs_status hs_run_presto(hs_plan_t plan, const float* d_spectra, const float* d_i
     HS_CUDA(guard.err);
     HsIO io{d_spectra, d_inv_baseline, d_snr, d_best_h, nullptr};
     return launch_presto(plan, plan->shape, st, io, (cudaStream_t)cuda_stream);
+}
+
+hs_status hs_run_greedy_dstats(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline, const float* d_mu,
+                               const float* d_sigma, float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream) {
+    hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, d_path);
+    if (rc != HS_OK) return rc;
+    if (!d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
+    HsStats st;
+    std::memset(&st, 0, sizeof(st));
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    HsIO io{d_spectra, d_inv_baseline, d_snr, d_best_h, d_path, d_mu, d_sigma};
+    return launch_greedy(plan, plan->shape, st, io, (cudaStream_t)cuda_stream);
+}
+
+hs_status hs_run_presto_dstats(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline, const float* d_mu,
+                               const float* d_sigma, float* d_snr, int32_t* d_best_h, void* cuda_stream) {
+    hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, nullptr);
+    if (rc != HS_OK) return rc;
+    if (!d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
+    HsStats st;
+    std::memset(&st, 0, sizeof(st));
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    HsIO io{d_spectra, d_inv_baseline, d_snr, d_best_h, nullptr, d_mu, d_sigma};
+    return launch_presto(plan, plan->shape, st, io, (cudaStream_t)cuda_stream);
+}
+
+int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip) {
+    if (!plan || n_clip < 0 || n_clip > 16) return -1;
+    return (int64_t)(n_clip + 1) * plan->shape.n_spectra * HS_MAX_H * 3 * (int64_t)sizeof(double);
+}
+
+hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
+                            int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
+                            float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream) {
+    if (!plan || !d_spectra || !d_mu || !d_sigma || !d_work) return HS_ERR_INVALID_ARG;
+    const HsShape& sh = plan->shape;
+    if (n_hi == 0) n_hi = sh.n_bins;
+    if (n_lo < 0 || n_hi > sh.n_bins || n_lo > n_hi || n_clip < 0 || n_clip > 16 || !(clip_sigma > 0.f)) return HS_ERR_INVALID_ARG;
+    if (!aligned16(d_spectra) || (d_inv_baseline && !aligned16(d_inv_baseline)) || (reinterpret_cast<uintptr_t>(d_work) & 7u) ||
+        (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u))
+        return HS_ERR_INVALID_ARG;
+    const int64_t need = hs_stats_workspace_bytes(plan, n_clip);
+    if (work_bytes < need) return HS_ERR_INVALID_ARG;
+    if (!greedy && !presto_flags_ok(sh.flags)) return HS_ERR_INVALID_ARG;
+    if (sh.n_bins >= (1ll << 31) - 64 - 1 && !greedy) return HS_ERR_UNSUPPORTED;
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    HS_CUDA(cudaMemsetAsync(d_work, 0, (size_t)need, stream));
+    double* acc = static_cast<double*>(d_work);
+    const long long per_round = (long long)sh.n_spectra * HS_MAX_H * 3;
+    const long long count = n_hi - n_lo;
+    if (count > 0) {
+        for (int r = 0; r <= n_clip; ++r) {
+            for (long long s0 = 0; s0 < sh.n_spectra; s0 += HS_MAX_GRID_Y) {
+                HsShape sub = sh;
+                sub.n_spectra = (int)std::min<long long>(HS_MAX_GRID_Y, sh.n_spectra - s0);
+                HsIO io{d_spectra + s0 * sh.in_stride, d_inv_baseline ? d_inv_baseline + s0 * sh.in_stride : nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+                HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, r ? acc + (r - 1) * per_round + s0 * HS_MAX_H * 3 : nullptr,
+                              acc + r * per_round + s0 * HS_MAX_H * 3};
+                dim3 grid((unsigned)((count + 255) / 256), (unsigned)sub.n_spectra);
+                if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                else if (greedy) hs_stats_pass_kernel<true, false><<<grid, 256, 0, stream>>>(sub, io, a);
+                else if (d_inv_baseline) hs_stats_pass_kernel<false, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                else hs_stats_pass_kernel<false, false><<<grid, 256, 0, stream>>>(sub, io, a);
+                plan->launches += 1;
+                HS_CUDA(cudaGetLastError());
+            }
+        }
+    }
+    const int total = sh.n_spectra * sh.H;
+    hs_stats_finish_kernel<<<(total + 255) / 256, 256, 0, stream>>>(acc + n_clip * per_round, sh.n_spectra, sh.H, d_mu, d_sigma);
+    plan->launches += 1;
+    plan->last_kernel = "hs_stats_pass_kernel";
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
 }
 
 hs_status hs_run_greedy_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline, const float* mu,

@@ -31,6 +31,8 @@ struct HsIO {
     float* __restrict__ snr;             // [S][out_stride]
     int* __restrict__ best_h;            // [S][out_stride]
     unsigned* __restrict__ path;         // nullable (greedy only)
+    const float* __restrict__ d_mu;      // nullable: per-spectrum statistics [S][H] on the device (hs_run_*_dstats);
+    const float* __restrict__ d_sigma;   //           then the by-value HsStats is not used
 };
 
 // flag values (mirrors include/hs.h; csrc includes hs.h in hs_api.cu and static_asserts equality)
@@ -51,3 +53,19 @@ __device__ __forceinline__ float hs_snr(float sum, float nmis, float inv_sigma) 
 __device__ __forceinline__ void st_cs(float* p, float v) { __stcs(p, v); }
 __device__ __forceinline__ void st_cs(int* p, int v) { __stcs(p, v); }
 __device__ __forceinline__ void st_cs(unsigned* p, unsigned v) { __stcs(p, v); }
+
+// Per-spectrum statistics (hs_run_*_dstats): the CTA forms the two constants of spectrum s from d_mu / d_sigma exactly
+// as the host does for the by-value statistics (IEEE reciprocal, one fp32 multiply) and keeps them in shared memory.
+// Must be called by every thread of the CTA.
+__device__ __forceinline__ void hs_load_dstats(HsStats& s_st, const HsIO& io, int s, int H) {
+    if (threadIdx.x < HS_MAX_H) {
+        float is = 1.f, nm = 0.f;
+        if ((int)threadIdx.x < H) {
+            is = __fdiv_rn(1.0f, __ldg(io.d_sigma + (long long)s * H + threadIdx.x));
+            nm = -__fmul_rn(__ldg(io.d_mu + (long long)s * H + threadIdx.x), is);
+        }
+        s_st.inv_sigma[threadIdx.x] = is;
+        s_st.nmis[threadIdx.x] = nm;
+    }
+    __syncthreads();
+}

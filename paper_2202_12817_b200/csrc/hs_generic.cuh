@@ -13,10 +13,13 @@ __device__ __forceinline__ float hs_load(const float* __restrict__ x, const floa
 }
 
 // Alg. 2, eq. 5.
-template <bool HAS_BASE>
+template <bool HAS_BASE, bool DSTATS = false>
 __global__ void __launch_bounds__(256)
-hs_greedy_generic_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
+hs_greedy_generic_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     const int s = blockIdx.y;
+    __shared__ HsStats s_st;
+    if (DSTATS) hs_load_dstats(s_st, io, s, sh.H);
+    const HsStats& st = DSTATS ? s_st : st_param;
     const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= sh.n_fund) return;
     const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
@@ -49,10 +52,13 @@ hs_greedy_generic_kernel(const __grid_constant__ HsShape sh, const __grid_consta
 }
 
 // Alg. 1, eq. 4, and the _all / + variants.
-template <bool HAS_BASE>
+template <bool HAS_BASE, bool DSTATS = false>
 __global__ void __launch_bounds__(256)
-hs_presto_generic_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
+hs_presto_generic_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     const int s = blockIdx.y;
+    __shared__ HsStats s_st;
+    if (DSTATS) hs_load_dstats(s_st, io, s, sh.H);
+    const HsStats& st = DSTATS ? s_st : st_param;
     const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= sh.n_fund) return;
     const float* __restrict__ x = io.x + (long long)s * sh.in_stride;

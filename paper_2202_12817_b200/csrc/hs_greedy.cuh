@@ -33,10 +33,14 @@ __host__ __device__ constexpr int mixed_grid(int nt) { return NBAND * ((nt + NBA
 
 // HAS_BASE: every x[b] is the fp32 product x[b] * inv_baseline[b] (reading R13; cfg4's whitening multiplier).
 // DRIFT = false: the simple harmonic sum (eq. 3; HS_GREEDY_NO_DRIFT): the second bin is never read.
-template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true, bool MIX = true>
+// DSTATS: per-spectrum statistics from device memory (hs_run_greedy_dstats) instead of the by-value ones.
+template <int BLOCK, int R, bool FUND_SELECT, bool WANT_PATH, bool HAS_BASE = false, bool DRIFT = true, bool MIX = true, bool DSTATS = false>
 __global__ void __launch_bounds__(BLOCK, (R == 4) ? 1536 / BLOCK : 1)
-hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
+hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     const int s = blockIdx.y;
+    __shared__ HsStats s_st;
+    if (DSTATS) hs_load_dstats(s_st, io, s, sh.H);
+    const HsStats& st = DSTATS ? s_st : st_param;
     const int N = (int)sh.n_bins;
     const int last = N - 1;
     const int n_fund = (int)sh.n_fund;

@@ -216,10 +216,13 @@ __device__ __forceinline__ void store8(float* __restrict__ ps, int* __restrict__
 }  // namespace hs_tile
 
 // grid: (tiles of 512 W outputs, spectra); block: 64 W threads; dynamic shared memory: 4 smem_words(L, W) bytes
-template <int L, int W>
+template <int L, int W, bool DSTATS = false>
 __global__ void __launch_bounds__(64 * W)
-hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st, HsIO io) {
+hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     using namespace hs_tile;
+    __shared__ HsStats s_st;
+    if (DSTATS) hs_load_dstats(s_st, io, blockIdx.y, sh.H);
+    const HsStats& st = DSTATS ? s_st : st_param;
     constexpr int NF = n_frac(L);
     extern __shared__ float4 hs_tile_smem4[];
     float* sm = reinterpret_cast<float*>(hs_tile_smem4);

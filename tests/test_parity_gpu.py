@@ -629,3 +629,114 @@ def test_cfg4_full_size(hs, oracle_mod):
     rows = [0, 511, 512, S - 1]
     check_greedy(oracle_mod, x[rows].cpu().numpy(), H, mu, sg, 0, out[0][rows].cpu().numpy(), out[1][rows].cpu().numpy(),
                  out[2][rows].cpu().numpy(), inv_baseline=ib[rows].cpu().numpy(), T=10.0)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-2: hs_estimate_stats (reading R14 of GetMeanStdev) and the per-spectrum statistics entry points
+# ------------------------------------------------------------------------------------------
+def _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, clip, n_clip, inv_baseline=None):
+    S, N = x.shape
+    istr = (N + 3) & ~3
+    dx = torch.zeros((S, istr), dtype=torch.float32, device="cuda")
+    dx[:, :N] = torch.as_tensor(x).cuda()
+    db = None
+    if inv_baseline is not None:
+        db = torch.ones((S, istr), dtype=torch.float32, device="cuda")
+        db[:, :N] = torch.as_tensor(inv_baseline).cuda()
+    mu = torch.full((S, H), float("nan"), dtype=torch.float32, device="cuda")
+    sg = torch.full((S, H), float("nan"), dtype=torch.float32, device="cuda")
+    plan = hs.hs_plan(N, S, H, istr, istr, 0, flags, 0)
+    try:
+        work = torch.empty(hs.hs_stats_workspace_bytes(plan, n_clip) // 8, dtype=torch.float64, device="cuda")
+        hs.hs_estimate_stats(plan, greedy, dx, db, n_lo, n_hi, clip, n_clip, mu, sg, work)
+        torch.cuda.synchronize()
+        last = work.view(n_clip + 1, S, 32, 3)[n_clip, :, :H, 0].cpu().numpy().astype(np.int64)
+    finally:
+        hs.hs_destroy(plan)
+    return mu.cpu().numpy(), sg.cpu().numpy(), last
+
+
+@pytest.mark.parametrize("greedy,flags", [(True, 0), (True, NO_FUND_SELECT), (True, NO_DRIFT), (False, 0),
+                                          (False, ALL_HARMONICS), (False, ALL_HARMONICS | ALL_ORDERS)])
+def test_estimate_stats_exact_integer(hs, oracle_mod, greedy, flags):
+    """Exact-integer spectra: the fp32 partial sums equal the oracle's fp64 ones, every fp64 moment is an exact
+    integer sum whatever the order of the additions, so counts, means and deviations must equal the oracle's exactly,
+    rounds of outlier rejection included; the range crosses the greedy band edges."""
+    H, S, N = 13, 3, 50001
+    x = inputs.integer_spectra(81, S, N, 40).numpy()
+    x[:, ::501] += 3000.0                                  # outliers for the rejection rounds
+    for n_lo, n_hi, n_clip in ((0, N, 0), (77, 9000, 2), (1000, 1001, 0), (5, 5, 1)):
+        mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, H, flags, greedy, n_lo, n_hi, clip=2.5, n_clip=n_clip)
+        mu, sg, cnt = _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, 2.5, n_clip)
+        assert np.array_equal(cnt, cnt_r), (n_lo, n_hi, n_clip)
+        assert np.array_equal(mu, mu_r) and np.array_equal(sg, sg_r), (n_lo, n_hi, n_clip)
+
+
+def test_estimate_stats_red_noise_and_dstats_run(hs, oracle_mod):
+    """cfg4 content at reduced size: statistics of the whitened greedy sums with two rejection rounds against the
+    oracle (fp32 vs fp64 partial sums: relative 1e-5; a sum within rounding of a limit may be kept on one side only),
+    then hs_run_greedy_dstats / hs_run_presto_dstats with per-spectrum statistics against the oracle run row by row."""
+    from parity import check_greedy, check_presto
+    H = 32
+    w = inputs.Workload("red", 3, 1 << 17, H, seed=4, n_pulsars=2, r_range=(100.0, 4000.0), duty_range=(0.02, 0.1),
+                        amp_range=(8.0, 12.0), red_noise=True)
+    xt = inputs.generate(w)
+    ib = inputs.block_median_inv_baseline(xt).numpy()
+    x = xt.numpy()
+    S, N = x.shape
+    n_lo, n_hi = N // 64, N // 32
+    for greedy in (True, False):
+        mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, H, 0, greedy, n_lo, n_hi, clip=3.0, n_clip=2, inv_baseline=ib)
+        mu, sg, cnt = _gpu_stats(hs, x, H, 0, greedy, n_lo, n_hi, 3.0, 2, inv_baseline=ib)
+        assert np.all(np.abs(cnt - cnt_r) <= 2)
+        assert np.allclose(mu, mu_r, rtol=1e-5, atol=0) and np.allclose(sg, sg_r, rtol=1e-4, atol=0)
+        if greedy:      # whitened noise: each step adds about the larger of two Exp(1) (SURVEY.md 8(c))
+            h = np.arange(1, H + 1)
+            assert np.all(np.abs(mu / (1.5 * h) - 1.0) < 0.1)
+        # the estimated statistics drive the run: per-spectrum mu / sigma from device memory
+        dmu, dsg = torch.from_numpy(mu).cuda(), torch.from_numpy(sg).cuda()
+        dx, db = torch.from_numpy(x).cuda(), torch.from_numpy(ib).cuda()
+        for tune in (0, GENERIC):
+            snr = torch.empty((S, N), dtype=torch.float32, device="cuda")
+            bh = torch.empty((S, N), dtype=torch.int32, device="cuda")
+            path = torch.empty((S, N), dtype=torch.int32, device="cuda")
+            plan = hs.hs_plan(N, S, H)
+            try:
+                hs.hs_plan_set_tuning(plan, tune)
+                if greedy:
+                    hs.hs_run_greedy_dstats(plan, dx, db, dmu, dsg, snr, bh, path)
+                else:
+                    hs.hs_run_presto_dstats(plan, dx, db, dmu, dsg, snr, bh)
+                torch.cuda.synchronize()
+            finally:
+                hs.hs_destroy(plan)
+            for s in range(S):
+                if greedy:
+                    check_greedy(oracle_mod, x[s:s + 1], H, mu[s], sg[s], 0, snr[s:s + 1].cpu().numpy(), bh[s:s + 1].cpu().numpy(),
+                                 path[s:s + 1].cpu().numpy(), inv_baseline=ib[s:s + 1], T=10.0)
+                else:
+                    check_presto(oracle_mod, x[s:s + 1], H, mu[s], sg[s], 0, snr[s:s + 1].cpu().numpy(), bh[s:s + 1].cpu().numpy(),
+                                 inv_baseline=ib[s:s + 1], T=10.0)
+
+
+def test_dstats_equals_by_value_statistics(hs, oracle_mod):
+    """The same statistics for every spectrum through the device arrays and through the host arrays: identical bits
+    (tile kernels without the multiplier, all tile shapes of the by-value path are the default one here)."""
+    H, S, N = 32, 4, 70004                                  # rows start on odd 16-byte units
+    x = inputs.generate(inputs.Workload("n", S, N, H, seed=12)).cuda()
+    out = [torch.empty((S, N + 4), dtype=torch.float32 if k % 2 == 0 else torch.int32, device="cuda") for k in range(4)]
+    plan = hs.hs_plan(N, S, H, N, N + 4, 0, 0, 0)
+    try:
+        for form in ("greedy", "presto"):
+            mu, sg = inputs.exp1_stats(form, H)
+            dmu, dsg = mu.repeat(S, 1).cuda(), sg.repeat(S, 1).cuda()
+            if form == "greedy":
+                hs.hs_run_greedy(plan, x, None, mu, sg, out[0], out[1], None)
+                hs.hs_run_greedy_dstats(plan, x, None, dmu, dsg, out[2], out[3], None)
+            else:
+                hs.hs_run_presto(plan, x, None, mu, sg, out[0], out[1])
+                hs.hs_run_presto_dstats(plan, x, None, dmu, dsg, out[2], out[3])
+            torch.cuda.synchronize()
+            assert torch.equal(out[0][:, :N].view(torch.int32), out[2][:, :N].view(torch.int32)) and torch.equal(out[1][:, :N], out[3][:, :N])
+    finally:
+        hs.hs_destroy(plan)
