@@ -58,6 +58,10 @@ def _load():
                                               c_d, c_i32, c_d]
         lib.hs_oracle_estimate_stats.argtypes = [c_f, c_f, i64, i32, i64, i32, u32, i32, i64, i64,
                                                  ctypes.c_double, i32, c_f, c_f, c_i64]
+        lib.hs_oracle_greedy_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, c_u32, i64, i32]
+        lib.hs_oracle_presto_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, i64, i32]
+        lib.hs_oracle_round_half_up.argtypes = [i64, i64]
+        lib.hs_oracle_round_half_up.restype = i64
         lib.hs_oracle_presto_index.argtypes = [i32, i32, i64]
         lib.hs_oracle_presto_index.restype = i64
         lib.hs_oracle_presto_order_in_set.argtypes = [i32, u32]
@@ -207,6 +211,41 @@ def estimate_stats(x, H: int, flags: int = 0, greedy: bool = True, n_lo: int = 0
     if rc != 0:
         raise ValueError("hs_oracle_estimate_stats: invalid arguments")
     return mu, sg, cnt
+
+
+def greedy_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None):
+    """R15: 2-D greedy (ours) / simple (NO_DRIFT) harmonic sum over a plane [n_z, N], n_z = 2 Z + 1.
+    Returns (snr float64, best_h int32, path uint32: bits 0-15 r-shifts, bits 16-31 z-shifts), each [n_z, N]."""
+    lib = _load()
+    a = _as_f32_2d(plane)
+    nz, N = a.shape
+    mu, sigma = _stats(mu, sigma, H)
+    snr = np.empty((nz, N), np.float64); bh = np.empty((nz, N), np.int32); path = np.empty((nz, N), np.uint32)
+    rc = lib.hs_oracle_greedy_2d(_ptr(a, ctypes.c_float), N, nz, N, H, _ptr(mu, ctypes.c_float), _ptr(sigma, ctypes.c_float), flags,
+                                 _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), _ptr(path, ctypes.c_uint32), N,
+                                 n_threads or host_threads())
+    if rc != 0:
+        raise ValueError("hs_oracle_greedy_2d: invalid arguments")
+    return snr, bh, path
+
+
+def presto_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None):
+    """R15: PRESTO-like 2-D harmonic sum, output indexed by the top harmonic (r, z).  Returns (snr, best_h)."""
+    lib = _load()
+    a = _as_f32_2d(plane)
+    nz, N = a.shape
+    mu, sigma = _stats(mu, sigma, H)
+    snr = np.empty((nz, N), np.float64); bh = np.empty((nz, N), np.int32)
+    rc = lib.hs_oracle_presto_2d(_ptr(a, ctypes.c_float), N, nz, N, H, _ptr(mu, ctypes.c_float), _ptr(sigma, ctypes.c_float), flags,
+                                 _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), N, n_threads or host_threads())
+    if rc != 0:
+        raise ValueError("hs_oracle_presto_2d: invalid arguments")
+    return snr, bh
+
+
+def round_half_up(a: int, b: int) -> int:
+    """Round(a / b), b > 0, as the 2-D oracle computes it (half up, also for negative a)."""
+    return int(_load().hs_oracle_round_half_up(a, b))
 
 
 def presto_index(h: int, Hp: int, n: int) -> int:

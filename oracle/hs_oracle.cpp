@@ -42,6 +42,15 @@
 //       count), followed by n_clip rounds of outlier rejection: round p keeps the sums with
 //       lo <= S_h(n) <= hi, lo/hi = mean -/+ clip * std of round p-1 rounded to fp32.  An order without samples gets
 //       (mu, sigma) = (0, 1); a zero standard deviation is returned as 1.
+//   R15 (NEXT-4, 2-D harmonic sum over the f-fdot plane; the paper only mentions it; BASELINE.json
+//       configs[4] gives S_h(r,z) = sum_{k<=h} P[round(k r), round(k z)]): the plane is P[z + Z][r], z in [-Z, Z];
+//       SIMPLE 2-D sum = that formula at integer (r, z); order k is evaluated iff k r <= N-1 and |k z| <= Z, and once an
+//       order is skipped all later ones are (as R4).  PRESTO-like 2-D: the output is indexed by the TOP harmonic (r, z)
+//       and the terms sit at (Round(k r / H'), Round(k z / H')), Round = round half up = floor((2a + b) / (2b)) also
+//       for negative z.  GREEDY 2-D is OURS (the paper defines no 2-D greedy rule): drifts d_r, d_z >= 0; at order h
+//       the candidates are the 2 x 2 block P[w..w+1][m..m+1], m = h r + d_r, w = h z + d_z; the largest is added (ties:
+//       the first of (m,w), (m+1,w), (m,w+1), (m+1,w+1)) and the drifts follow it; candidates outside the plane never
+//       win; path bit h-1 = r-shift at order h, bit 16+h-1 = z-shift (H <= 16).
 //   NEXT-2: an optional per-bin multiplier inv_baseline[] whitens the spectrum; the product
 //       x*inv_baseline is formed in fp32 (one IEEE multiply -- the kernel's precision --
 //       because it decides the greedy comparison), everything after it in fp64.
@@ -315,6 +324,89 @@ int hs_oracle_estimate_stats(const float* x, const float* inv_baseline, int64_t 
     }
     return 0;
 }
+
+// ---- R15: 2-D harmonic sums over an f-fdot plane P[n_z][stride], n_z = 2 Z + 1 (NEXT-4) ----------------------------
+namespace {
+inline int64_t floor_div(int64_t a, int64_t b) { int64_t q = a / b; if ((a % b != 0) && ((a < 0) != (b < 0))) --q; return q; }
+inline int64_t round_half_up(int64_t a, int64_t b) { return floor_div(2 * a + b, 2 * b); }   // Round(a / b), b > 0
+
+struct Plane {
+    const float* p; int64_t N, stride; int32_t Z;
+    double at(int64_t z, int64_t r) const { return (double)p[(z + Z) * stride + r]; }
+};
+
+void greedy2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64_t r, int64_t z,
+                  double* best_out, int32_t* besth_out, uint32_t* path_out) {
+    int64_t dr = 0, dz = 0;
+    double sum = 0.0, best = NEG_INF;
+    int32_t bh = 0;
+    uint32_t path = 0;
+    for (int h = 1; h <= H; ++h) {
+        const int64_t m = (int64_t)h * r + dr, w = (int64_t)h * z + dz;
+        if (m > pl.N - 1 || w < -pl.Z || w > pl.Z) break;
+        const bool drift = !(flags & F_NO_DRIFT) && !(h == 1 && (flags & F_NO_FUND_SELECT));
+        const bool r1 = drift && m + 1 <= pl.N - 1, z1 = drift && w + 1 <= pl.Z;
+        const double c[4] = {pl.at(w, m), r1 ? pl.at(w, m + 1) : NEG_INF, z1 ? pl.at(w + 1, m) : NEG_INF,
+                             (r1 && z1) ? pl.at(w + 1, m + 1) : NEG_INF};
+        int pick = 0;
+        for (int k = 1; k < 4; ++k) if (c[k] > c[pick]) pick = k;      // strict >: the first maximum stays
+        if (pick & 1) { dr += 1; path |= 1u << (h - 1); }
+        if (pick & 2) { dz += 1; path |= 1u << (16 + h - 1); }
+        sum += c[pick];
+        const double s = st.snr(sum, h);
+        if (s > best) { best = s; bh = h; }
+    }
+    *best_out = best; *besth_out = bh;
+    if (path_out) *path_out = path;
+}
+
+void presto2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64_t r, int64_t z,
+                  double* best_out, int32_t* besth_out) {
+    double best = NEG_INF;
+    int32_t bh = 0;
+    for (int Hp = 1; Hp <= H; ++Hp) {
+        if (!order_in_set(Hp, flags)) continue;
+        double sum = pl.at(round_half_up(z, Hp), round_half_up(r, Hp));
+        const int step = (flags & F_ALL_HARMONICS) ? 1 : 2;
+        for (int k = 2; k <= Hp; k += step) sum += pl.at(round_half_up((int64_t)k * z, Hp), round_half_up((int64_t)k * r, Hp));
+        const double s = st.snr(sum, Hp);
+        if (s > best) { best = s; bh = Hp; }
+    }
+    *best_out = best; *besth_out = bh;
+}
+}  // namespace
+
+// plane: [n_z][stride] fp32, n_z odd; outputs [n_z][out_stride]; H <= 16.  Returns 0, or 1 on invalid arguments.
+int hs_oracle_greedy_2d(const float* plane, int64_t N, int32_t n_z, int64_t stride, int32_t H, const float* mu, const float* sigma,
+                        uint32_t flags, double* snr, int32_t* best_h, uint32_t* path, int64_t out_stride, int32_t n_threads) {
+    if (bad_common(plane, N, n_z, H, mu, sigma) || H > 16 || !(n_z & 1) || !snr || !best_h || stride < N || out_stride < N) return 1;
+    const Stats st{mu, sigma};
+    const Plane pl{plane, N, stride, (n_z - 1) / 2};
+    parallel_for_rows(n_z, N, n_threads, [&](int32_t zi, int64_t lo, int64_t hi) {
+        for (int64_t r = lo; r < hi; ++r) {
+            const int64_t o = (int64_t)zi * out_stride + r;
+            greedy2d_bin(pl, H, st, flags, r, (int64_t)zi - pl.Z, &snr[o], &best_h[o], path ? &path[o] : nullptr);
+        }
+    });
+    return 0;
+}
+
+int hs_oracle_presto_2d(const float* plane, int64_t N, int32_t n_z, int64_t stride, int32_t H, const float* mu, const float* sigma,
+                        uint32_t flags, double* snr, int32_t* best_h, int64_t out_stride, int32_t n_threads) {
+    if (bad_common(plane, N, n_z, H, mu, sigma) || H > 16 || !(n_z & 1) || !snr || !best_h || stride < N || out_stride < N) return 1;
+    if ((flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    const Stats st{mu, sigma};
+    const Plane pl{plane, N, stride, (n_z - 1) / 2};
+    parallel_for_rows(n_z, N, n_threads, [&](int32_t zi, int64_t lo, int64_t hi) {
+        for (int64_t r = lo; r < hi; ++r) {
+            const int64_t o = (int64_t)zi * out_stride + r;
+            presto2d_bin(pl, H, st, flags, r, (int64_t)zi - pl.Z, &snr[o], &best_h[o]);
+        }
+    });
+    return 0;
+}
+
+int64_t hs_oracle_round_half_up(int64_t a, int64_t b) { return round_half_up(a, b); }
 
 // Index helpers exposed so the pins can check them against the paper's worked example
 // (bin 800 is the last element of fundamental 100 at H = 8 and of 200 at H = 4).

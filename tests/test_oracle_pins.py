@@ -599,3 +599,117 @@ def test_r14_stats_closed_forms_and_degenerate_cases(oracle_mod):
     c = np.full((1, 5000), 3.0, np.float32)
     mu, sg, cnt = oracle_mod.estimate_stats(c, 8, 0, True, 10, 500)
     assert np.array_equal(mu[0], 3.0 * np.arange(1, 9)) and np.all(sg == 1.0)
+
+
+# ------------------------------------------------------------------------------------------
+# R15 (NEXT-4): 2-D harmonic sums over an f-fdot plane -- oracle.greedy_2d / oracle.presto_2d
+# ------------------------------------------------------------------------------------------
+def _int_plane(seed, nz, N, max_val=50):
+    return inputs.integer_spectra(seed, nz, N, max_val).numpy()
+
+
+def test_r15_round_half_up_exact_rational(oracle_mod):
+    from fractions import Fraction
+    for b in (1, 2, 3, 4, 8, 16):
+        for a in range(-70, 71):
+            assert oracle_mod.round_half_up(a, b) == math.floor(Fraction(a, b) + Fraction(1, 2)), (a, b)
+
+
+def test_r15_row_z0_reproduces_the_1d_sums(oracle_mod):
+    """z = 0: k z = 0 for every k, so the 2-D simple sum and the 2-D PRESTO-like sums of that row are the 1-D sums of
+    the row P[Z] (bit for bit: same terms in the same order)."""
+    H, nz, N = 16, 7, 5000
+    P = _int_plane(5, nz, N)
+    Z = nz // 2
+    mu, sg = (np.arange(1, H + 1, dtype=np.float32) * 3, np.sqrt(np.arange(1, H + 1)).astype(np.float32))
+    s2, b2, p2 = oracle_mod.greedy_2d(P, H, mu, sg, NO_DRIFT)
+    s1, b1, p1 = oracle_mod.greedy(P[Z], H, mu, sg, NO_DRIFT)
+    assert np.array_equal(s2[Z], s1[0]) and np.array_equal(b2[Z], b1[0]) and not p2.any()
+    for flags in (0, ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS):
+        s2, b2 = oracle_mod.presto_2d(P, H, mu, sg, flags)
+        s1, b1 = oracle_mod.presto(P[Z], H, mu, sg, flags)
+        assert np.array_equal(s2[Z], s1[0]) and np.array_equal(b2[Z], b1[0])
+
+
+def test_r15_brute_force_tiny_plane(oracle_mod):
+    """Independent restatement in plain Python (exact rational rounding, argmax over an explicit candidate list)."""
+    from fractions import Fraction
+    H, nz, N = 6, 9, 40
+    Z = nz // 2
+    P = _int_plane(6, nz, N, 9).astype(np.float64)
+    mu = np.array([2.0 * h for h in range(1, H + 1)], np.float32)
+    sg = np.array([2.0 ** (h % 3) for h in range(1, H + 1)], np.float32)
+    rnd = lambda a, b: math.floor(Fraction(a, b) + Fraction(1, 2))
+    for flags in (0, NO_FUND_SELECT, NO_DRIFT):
+        s, b, p = oracle_mod.greedy_2d(P.astype(np.float32), H, mu, sg, flags)
+        for z in range(-Z, Z + 1):
+            for r in range(N):
+                dr = dz = 0; tot = 0.0; best = -math.inf; bh = 0; path = 0
+                for h in range(1, H + 1):
+                    m, w = h * r + dr, h * z + dz
+                    if m > N - 1 or abs(w) > Z:
+                        break
+                    cand = [(P[w + Z, m], 0, 0)]
+                    if not (flags & NO_DRIFT) and not (h == 1 and flags & NO_FUND_SELECT):
+                        if m + 1 < N: cand.append((P[w + Z, m + 1], 1, 0))
+                        if w + 1 <= Z: cand.append((P[w + 1 + Z, m], 0, 1))
+                        if m + 1 < N and w + 1 <= Z: cand.append((P[w + 1 + Z, m + 1], 1, 1))
+                    v, sr, sz = max(cand, key=lambda t: t[0])          # max() keeps the first of equal values
+                    dr += sr; dz += sz; tot += v
+                    path |= (sr << (h - 1)) | (sz << (16 + h - 1))
+                    snr = (tot - float(mu[h - 1])) / float(sg[h - 1])
+                    if snr > best: best, bh = snr, h
+                assert (s[z + Z, r], b[z + Z, r], p[z + Z, r]) == (best, bh, path), (flags, z, r)
+    for flags in (0, ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS):
+        s, b = oracle_mod.presto_2d(P.astype(np.float32), H, mu, sg, flags)
+        orders = [Hp for Hp in range(1, H + 1) if flags & ALL_ORDERS or Hp & (Hp - 1) == 0]
+        for z in range(-Z, Z + 1):
+            for r in range(N):
+                best, bh = -math.inf, 0
+                for Hp in orders:
+                    ks = range(1, Hp + 1) if flags & ALL_HARMONICS else [1] + list(range(2, Hp + 1, 2))
+                    tot = sum(P[rnd(k * z, Hp) + Z, rnd(k * r, Hp)] for k in ks)
+                    snr = (tot - float(mu[Hp - 1])) / float(sg[Hp - 1])
+                    if snr > best: best, bh = snr, Hp
+                assert (s[z + Z, r], b[z + Z, r]) == (best, bh), (flags, z, r)
+
+
+def test_r15_drifting_delta_train_and_truncation(oracle_mod):
+    """A train of K deltas at (k r0, k z0) (BASELINE.json configs[4]: S_h(r,z) = sum P[k r, k z]): the simple 2-D sum
+    peaks at (r0, z0) with best_h = K and snr (A-1) sqrt(K); at fractional (r0 + e, z0 + f) the bins are
+    (floor(k (r0 + e)), floor(k (z0 + f))) and the 2-D greedy rule follows them; PRESTO_all 2-D peaks at the top
+    harmonic (K r0, K z0).  Constant plane: best_h = number of evaluated orders = min(H, (N-1)//r, Z//|z|)."""
+    H, nz, N, K, A = 16, 41, 3000, 8, 10.0
+    Z = nz // 2
+    mu = np.arange(1, H + 1, dtype=np.float32)
+    sg = np.sqrt(np.arange(1, H + 1)).astype(np.float32)
+    r0, z0 = 150, -2
+    P = np.zeros((nz, N), np.float32)
+    for k in range(1, K + 1):
+        P[k * z0 + Z, k * r0] = A
+    s, b, p = oracle_mod.greedy_2d(P, H, mu, sg, NO_DRIFT)
+    assert (np.unravel_index(np.argmax(s), s.shape)) == (z0 + Z, r0) and b[z0 + Z, r0] == K
+    assert abs(s[z0 + Z, r0] - (A - 1) * math.sqrt(K)) < 1e-5           # sigma is the fp32 sqrt
+    s, b = oracle_mod.presto_2d(P, H, mu, sg, ALL_HARMONICS)
+    assert (np.unravel_index(np.argmax(s), s.shape)) == (K * z0 + Z, K * r0) and b[K * z0 + Z, K * r0] == K
+    e, f = 0.37, 0.55
+    P = np.zeros((nz, N), np.float32)
+    want = 0
+    for k in range(1, K + 1):
+        P[math.floor(k * (z0 + f)) + Z, math.floor(k * (r0 + e))] = A
+    for k in range(1, K + 1):
+        if math.floor(k * e) > math.floor((k - 1) * e): want |= 1 << (k - 1)
+        if math.floor(k * f) > math.floor((k - 1) * f): want |= 1 << (16 + k - 1)
+    s, b, p = oracle_mod.greedy_2d(P, H, mu, sg, 0)
+    assert b[z0 + Z, r0] == K and abs(s[z0 + Z, r0] - (A - 1) * math.sqrt(K)) < 1e-5
+    assert (p[z0 + Z, r0] & ((1 << K) - 1 | ((1 << K) - 1) << 16)) == want
+    sS, _, _ = oracle_mod.greedy_2d(P, H, mu, sg, NO_DRIFT)
+    assert sS[z0 + Z, r0] < s[z0 + Z, r0]                       # the simple sum loses the drifting harmonics
+    C = np.full((nz, N), 3.0, np.float32)
+    s, b, p = oracle_mod.greedy_2d(C, H, mu, sg, 0)
+    assert not p.any()                                          # ties stay on the first candidate
+    for z in (-20, -7, -1, 0, 3, 20):
+        for r in (0, 1, 100, 187, 1499, 2999):
+            n_r = H if r == 0 else min(H, (N - 1) // r)
+            n_z = H if z == 0 else min(H, Z // abs(z))
+            assert b[z + Z, r] == min(n_r, n_z), (z, r)
