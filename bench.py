@@ -479,8 +479,112 @@ def run_cuda(args):
     return 0
 
 
+def run_cuda_2d(args):
+    """--workload cfg5 (BASELINE.json configs[4], NEXT-4): one f-fdot plane, 201 x 2^21 bins, H = 16; a step =
+    hs_run_greedy_2d (the 2-D greedy rule of reading R15) + hs_run_presto_2d on the same plane.  1 GPU."""
+    import torch
+    from paper_2202_12817_b200 import binding as hs
+    from paper_2202_12817_b200 import inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    hs.load()
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    w = inputs.plane_workload(args.workload)
+    nz, N, H = w.n_z, w.n_bins, (args.H or w.H)
+    P = inputs.generate_plane(w, dev)
+    snr_g = torch.empty((nz, N), dtype=torch.float32, device=dev); bh_g = torch.empty((nz, N), dtype=torch.int32, device=dev)
+    snr_p = torch.empty_like(snr_g); bh_p = torch.empty_like(bh_g)
+    gv, fs, pv = _variants(args)
+    mu_g, sg_g = inputs.exp1_stats("simple", H)
+    mu_p, sg_p = inputs.exp1_stats(pv, H)
+    plan_g = hs.hs_plan_2d(N, nz, H, flags=args.greedy_flags, device=0)
+    plan_p = hs.hs_plan_2d(N, nz, H, flags=args.presto_flags, device=0)
+    stream = torch.cuda.current_stream(dev)
+    do_g, do_p = args.forms != "presto", args.forms != "greedy"
+
+    def step(ev=None):
+        if ev is not None:
+            ev[0].record(stream)
+        if do_g:
+            hs.hs_run_greedy_2d(plan_g, P, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
+        if ev is not None:
+            ev[1].record(stream)
+        if do_p:
+            hs.hs_run_presto_2d(plan_p, P, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
+        if ev is not None:
+            ev[2].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    l0 = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p)
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        step(evs[k])
+    torch.cuda.synchronize()
+    launches = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p) - l0
+    total_ms = evs[0][0].elapsed_time(evs[-1][2])
+    g_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    p_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    t_end = time.time() + 1.0
+    while time.time() < t_end:
+        step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    peak, peak_src = measured_peak()
+    bins = float(nz) * N
+    alg_bytes = BYTES_PER_BIN * bins
+
+    def per_kernel(name, ms):
+        a = alg_bytes / (ms * 1e-3) / 1e9
+        return {"kernel": name, "launch_ms": ms, "achieved": a, "frac": a / peak, "gbins_per_s": bins / ms / 1e6, "traffic": None}
+
+    pk = {}
+    if do_g:
+        pk["greedy_2d"] = per_kernel(hs.hs_last_kernel(plan_g), g_ms)
+    if do_p:
+        pk["presto_2d"] = per_kernel(hs.hs_last_kernel(plan_p), p_ms)
+    dom = max(pk, key=lambda k: pk[k]["launch_ms"])
+    cpu = None
+    if not args.no_cpu:
+        import oracle
+        oracle.build()
+        rows = (98, 102)                                   # z = -2 .. 1: rows where all 16 orders exist
+        Ph = P.cpu().numpy()
+        t0 = time.perf_counter()
+        if do_g:
+            oracle.greedy_2d(Ph, H, mu_g.numpy(), sg_g.numpy(), args.greedy_flags, rows=rows)
+        if do_p:
+            oracle.presto_2d(Ph, H, mu_p.numpy(), sg_p.numpy(), args.presto_flags, rows=rows)
+        dt = time.perf_counter() - t0
+        cpu = {"value": (rows[1] - rows[0]) * N / dt, "unit": UNIT, "cores": oracle.host_threads(), "kind": "oracle",
+               "sample": f"rows z = -2 .. 1 of the plane (4 x {N} bins, all 16 orders evaluated), fp64"}
+    hs.hs_destroy(plan_g); hs.hs_destroy(plan_p)
+    line = {"metric": "2-D harmonic-sum plane bins/s at H=16 (greedy-2D + PRESTO-like-2D forms per bin)", "value": bins * args.steps / (total_ms * 1e-3),
+            "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{w.name}: one f-fdot plane, {nz} rows (z = -{(nz - 1) // 2}..{(nz - 1) // 2}) x {N} fp32 bins, H={H}, "
+                                   f"{len(w.signals)} drifting signals; reading R15 (the 2-D greedy rule is this repository's, not the paper's)",
+                       "seed": w.seed, "l2": f"plane ({nz * N * 4 / 2**30:.2f} GiB) exceeds L2; no flush needed"},
+            "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": dom, "kernel_name": pk[dom]["kernel"], "achieved": pk[dom]["achieved"], "peak": peak,
+                         "unit": "GB/s", "frac": pk[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": pk[dom]["launch_ms"], "per_kernel": pk},
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     args = parse_args()
+    if args.workload == "cfg5":
+        if args.impl == "reference" or args.gpus > 1:
+            raise SystemExit("bench.py: --workload cfg5 (NEXT-4) is a 1-GPU, CUDA-arm workload")
+        return run_cuda_2d(args)
     if args.impl == "reference":
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

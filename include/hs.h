@@ -178,6 +178,30 @@ hs_status hs_run_both_host(hs_plan_t plan, const float* h_spectra, const float* 
                            const float* mu_presto, const float* sigma_presto,
                            float* h_snr_presto, int32_t* h_best_h_presto);
 
+/* NEXT-4: 2-D harmonic sums over an f-fdot (acceleration) plane (BASELINE.json configs[4]; the paper only mentions
+ * higher-dimensional harmonic sums, and defines no algorithm for them).  Reading R15 of DESIGN.md:
+ * the plane is P[z + Z][r], z = -Z .. Z (n_z = 2 Z + 1 rows of n_bins fp32 powers, row stride in_stride); outputs are
+ * written for every (z, r) at [z + Z][r] (row stride out_stride).  H <= 16, n_bins <= 2^25, n_z odd.
+ *   hs_run_greedy_2d, plan flag HS_GREEDY_NO_DRIFT: the SIMPLE 2-D sum S_h(r, z) = sum_{k <= h} P[k z][k r]
+ *     (BASELINE.json's formula at integer (r, z)); order k is evaluated iff k r <= n_bins - 1 and |k z| <= Z, and once
+ *     an order is skipped all later ones are; snr_h = (S_h - mu[h-1]) / sigma[h-1], output = the first maximum over h.
+ *   hs_run_greedy_2d, no flag: a 2-D GREEDY rule, OURS (not the paper's): drifts d_r = d_z = 0; at order h let
+ *     m = h r + d_r, w = h z + d_z (stop if m > n_bins - 1 or |w| > Z); the candidates are P[w][m], P[w][m+1],
+ *     P[w+1][m], P[w+1][m+1] (those outside the plane never win; at h = 1 only P[w][m] under
+ *     HS_GREEDY_NO_FUND_SELECT); the largest is added, ties going to the first in that order, and d_r / d_z grow by
+ *     one if it lies at m+1 / w+1.  d_path (nullable): bit h-1 = r-shift at order h, bit 16+h-1 = z-shift.
+ *   hs_run_presto_2d: the PRESTO-like form: the output index (r, z) is the TOP harmonic; for H' in the order set
+ *     S = sum over k in {1} U {2,4,..,H'} (1..H' under HS_PRESTO_ALL_HARMONICS) of
+ *     P[Round(k z / H')][Round(k r / H')], Round(a / b) = floor((2a + b) / (2b)) (half up, also for negative z).
+ * mu, sigma: HOST arrays of H floats.  Asynchronous on the stream.  The 1-D entry points reject a 2-D plan and vice
+ * versa; hs_find_candidates accepts both (spectrum = z + Z). */
+hs_status hs_plan_2d(hs_plan_t* plan, int64_t n_bins, int32_t n_z, int32_t H,
+                     int64_t in_stride, int64_t out_stride, uint32_t flags, int32_t device);
+hs_status hs_run_greedy_2d(hs_plan_t plan, const float* d_plane, const float* mu, const float* sigma,
+                           float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream);
+hs_status hs_run_presto_2d(hs_plan_t plan, const float* d_plane, const float* mu, const float* sigma,
+                           float* d_snr, int32_t* d_best_h, void* cuda_stream);
+
 /* One detection (reading R11 of DESIGN.md: a bin whose maximum SNR reaches the threshold). */
 typedef struct {
     int32_t spectrum;   /* row s of the batch */

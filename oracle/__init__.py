@@ -58,8 +58,8 @@ def _load():
                                               c_d, c_i32, c_d]
         lib.hs_oracle_estimate_stats.argtypes = [c_f, c_f, i64, i32, i64, i32, u32, i32, i64, i64,
                                                  ctypes.c_double, i32, c_f, c_f, c_i64]
-        lib.hs_oracle_greedy_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, c_u32, i64, i32]
-        lib.hs_oracle_presto_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, i64, i32]
+        lib.hs_oracle_greedy_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, c_u32, i64, i32, i32, i32]
+        lib.hs_oracle_presto_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, i64, i32, i32, i32]
         lib.hs_oracle_round_half_up.argtypes = [i64, i64]
         lib.hs_oracle_round_half_up.restype = i64
         lib.hs_oracle_presto_index.argtypes = [i32, i32, i64]
@@ -213,31 +213,34 @@ def estimate_stats(x, H: int, flags: int = 0, greedy: bool = True, n_lo: int = 0
     return mu, sg, cnt
 
 
-def greedy_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None):
+def greedy_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None, rows: Optional[Tuple[int, int]] = None):
     """R15: 2-D greedy (ours) / simple (NO_DRIFT) harmonic sum over a plane [n_z, N], n_z = 2 Z + 1.
-    Returns (snr float64, best_h int32, path uint32: bits 0-15 r-shifts, bits 16-31 z-shifts), each [n_z, N]."""
+    Returns (snr float64, best_h int32, path uint32: bits 0-15 r-shifts, bits 16-31 z-shifts), each [n_z, N];
+    with rows = (lo, hi) only the rows lo <= z + Z < hi are computed (the others are left as NaN / 0)."""
     lib = _load()
     a = _as_f32_2d(plane)
     nz, N = a.shape
     mu, sigma = _stats(mu, sigma, H)
-    snr = np.empty((nz, N), np.float64); bh = np.empty((nz, N), np.int32); path = np.empty((nz, N), np.uint32)
+    lo, hi = rows if rows is not None else (0, nz)
+    snr = np.full((nz, N), np.nan, np.float64); bh = np.zeros((nz, N), np.int32); path = np.zeros((nz, N), np.uint32)
     rc = lib.hs_oracle_greedy_2d(_ptr(a, ctypes.c_float), N, nz, N, H, _ptr(mu, ctypes.c_float), _ptr(sigma, ctypes.c_float), flags,
                                  _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), _ptr(path, ctypes.c_uint32), N,
-                                 n_threads or host_threads())
+                                 n_threads or host_threads(), lo, hi)
     if rc != 0:
         raise ValueError("hs_oracle_greedy_2d: invalid arguments")
     return snr, bh, path
 
 
-def presto_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None):
+def presto_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None, rows: Optional[Tuple[int, int]] = None):
     """R15: PRESTO-like 2-D harmonic sum, output indexed by the top harmonic (r, z).  Returns (snr, best_h)."""
     lib = _load()
     a = _as_f32_2d(plane)
     nz, N = a.shape
     mu, sigma = _stats(mu, sigma, H)
-    snr = np.empty((nz, N), np.float64); bh = np.empty((nz, N), np.int32)
+    lo, hi = rows if rows is not None else (0, nz)
+    snr = np.full((nz, N), np.nan, np.float64); bh = np.zeros((nz, N), np.int32)
     rc = lib.hs_oracle_presto_2d(_ptr(a, ctypes.c_float), N, nz, N, H, _ptr(mu, ctypes.c_float), _ptr(sigma, ctypes.c_float), flags,
-                                 _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), N, n_threads or host_threads())
+                                 _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), N, n_threads or host_threads(), lo, hi)
     if rc != 0:
         raise ValueError("hs_oracle_presto_2d: invalid arguments")
     return snr, bh

@@ -376,13 +376,17 @@ void presto2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64
 }
 }  // namespace
 
-// plane: [n_z][stride] fp32, n_z odd; outputs [n_z][out_stride]; H <= 16.  Returns 0, or 1 on invalid arguments.
+// plane: [n_z][stride] fp32, n_z odd; outputs [n_z][out_stride], only rows zi_lo <= z + Z < zi_hi are computed and
+// written (the sums still read the whole plane); H <= 16.  Returns 0, or 1 on invalid arguments.
 int hs_oracle_greedy_2d(const float* plane, int64_t N, int32_t n_z, int64_t stride, int32_t H, const float* mu, const float* sigma,
-                        uint32_t flags, double* snr, int32_t* best_h, uint32_t* path, int64_t out_stride, int32_t n_threads) {
+                        uint32_t flags, double* snr, int32_t* best_h, uint32_t* path, int64_t out_stride, int32_t n_threads,
+                        int32_t zi_lo, int32_t zi_hi) {
     if (bad_common(plane, N, n_z, H, mu, sigma) || H > 16 || !(n_z & 1) || !snr || !best_h || stride < N || out_stride < N) return 1;
+    if (zi_lo < 0 || zi_hi > n_z || zi_lo > zi_hi) return 1;
     const Stats st{mu, sigma};
     const Plane pl{plane, N, stride, (n_z - 1) / 2};
-    parallel_for_rows(n_z, N, n_threads, [&](int32_t zi, int64_t lo, int64_t hi) {
+    parallel_for_rows(zi_hi - zi_lo, N, n_threads, [&](int32_t row, int64_t lo, int64_t hi) {
+        const int32_t zi = zi_lo + row;
         for (int64_t r = lo; r < hi; ++r) {
             const int64_t o = (int64_t)zi * out_stride + r;
             greedy2d_bin(pl, H, st, flags, r, (int64_t)zi - pl.Z, &snr[o], &best_h[o], path ? &path[o] : nullptr);
@@ -392,12 +396,15 @@ int hs_oracle_greedy_2d(const float* plane, int64_t N, int32_t n_z, int64_t stri
 }
 
 int hs_oracle_presto_2d(const float* plane, int64_t N, int32_t n_z, int64_t stride, int32_t H, const float* mu, const float* sigma,
-                        uint32_t flags, double* snr, int32_t* best_h, int64_t out_stride, int32_t n_threads) {
+                        uint32_t flags, double* snr, int32_t* best_h, int64_t out_stride, int32_t n_threads,
+                        int32_t zi_lo, int32_t zi_hi) {
     if (bad_common(plane, N, n_z, H, mu, sigma) || H > 16 || !(n_z & 1) || !snr || !best_h || stride < N || out_stride < N) return 1;
     if ((flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    if (zi_lo < 0 || zi_hi > n_z || zi_lo > zi_hi) return 1;
     const Stats st{mu, sigma};
     const Plane pl{plane, N, stride, (n_z - 1) / 2};
-    parallel_for_rows(n_z, N, n_threads, [&](int32_t zi, int64_t lo, int64_t hi) {
+    parallel_for_rows(zi_hi - zi_lo, N, n_threads, [&](int32_t row, int64_t lo, int64_t hi) {
+        const int32_t zi = zi_lo + row;
         for (int64_t r = lo; r < hi; ++r) {
             const int64_t o = (int64_t)zi * out_stride + r;
             presto2d_bin(pl, H, st, flags, r, (int64_t)zi - pl.Z, &snr[o], &best_h[o]);

@@ -26,7 +26,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
-           "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes",
+           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -69,6 +69,12 @@ def load() -> ctypes.CDLL:
     lib.hs_plan_set_tuning.restype = ctypes.c_int
     lib.hs_find_candidates.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp, vp]
     lib.hs_find_candidates.restype = ctypes.c_int
+    lib.hs_plan_2d.argtypes = [ctypes.POINTER(vp), i64, i32, i32, i64, i64, u32, i32]
+    lib.hs_plan_2d.restype = ctypes.c_int
+    lib.hs_run_greedy_2d.argtypes = [vp, vp, fp, fp, vp, vp, vp, vp]
+    lib.hs_run_greedy_2d.restype = ctypes.c_int
+    lib.hs_run_presto_2d.argtypes = [vp, vp, fp, fp, vp, vp, vp]
+    lib.hs_run_presto_2d.restype = ctypes.c_int
     lib.hs_run_greedy_dstats.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.hs_run_greedy_dstats.restype = ctypes.c_int
     lib.hs_run_presto_dstats.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
@@ -149,6 +155,33 @@ def hs_run_presto(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.
                              _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), _farr(mu), _farr(sigma),
                              _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
                              stream), "hs_run_presto")
+
+
+def hs_plan_2d(n_bins: int, n_z: int, H: int, in_stride: int = 0, out_stride: int = 0, flags: int = 0, device: int = 0) -> ctypes.c_void_p:
+    lib = load()
+    plan = ctypes.c_void_p()
+    _check(lib.hs_plan_2d(ctypes.byref(plan), n_bins, n_z, H, in_stride, out_stride, flags, device), "hs_plan_2d")
+    return plan
+
+
+def hs_run_greedy_2d(plan, d_plane: torch.Tensor, mu, sigma, d_snr: torch.Tensor, d_best_h: torch.Tensor,
+                     d_path: Optional[torch.Tensor] = None, stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_plane.device).cuda_stream
+    _check(lib.hs_run_greedy_2d(plan, _dptr(d_plane, torch.float32, "d_plane"), _farr(mu), _farr(sigma),
+                                _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
+                                _dptr(d_path, torch.int32, "d_path"), stream), "hs_run_greedy_2d")
+
+
+def hs_run_presto_2d(plan, d_plane: torch.Tensor, mu, sigma, d_snr: torch.Tensor, d_best_h: torch.Tensor,
+                     stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_plane.device).cuda_stream
+    _check(lib.hs_run_presto_2d(plan, _dptr(d_plane, torch.float32, "d_plane"), _farr(mu), _farr(sigma),
+                                _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"), stream),
+           "hs_run_presto_2d")
 
 
 def hs_run_greedy_dstats(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor], d_mu: torch.Tensor,

@@ -16,6 +16,7 @@
 #include "hs_presto_farey.cuh"
 #include "hs_candidates.cuh"
 #include "hs_stats.cuh"
+#include "hs_2d.cuh"
 
 static_assert(HS_GREEDY_NO_FUND_SELECT == HSF_NO_FUND_SELECT, "flag mismatch");
 static_assert(HS_GREEDY_NO_DRIFT == HSF_NO_DRIFT, "flag mismatch");
@@ -42,6 +43,7 @@ struct HostStage {          // staging for the *_host entry points (created on f
 struct hs_plan_s {
     HsShape shape;
     uint32_t tune;          // hs_plan_set_tuning (0 = the library's choice)
+    bool two_d;             // hs_plan_2d: the batch is one f-fdot plane (rows z = -Z .. Z)
     int device;
     int sm_count;
     int64_t launches;
@@ -333,7 +335,7 @@ struct HostForm {           // one form's host-side arguments (snr == nullptr: t
 // Spectra go through the plan's two staging slots in groups of rows: upload ONCE, run the requested forms on the
 // slot, download their outputs; the two slots alternate on two streams so copies and kernels overlap.
 hs_status run_host(hs_plan_s* p, const float* hx, const float* hb, const HostForm& gr, const HostForm& pr) {
-    if (!p || !hx || (!gr.snr && !pr.snr)) return HS_ERR_INVALID_ARG;
+    if (!p || p->two_d || !hx || (!gr.snr && !pr.snr)) return HS_ERR_INVALID_ARG;
     if ((gr.snr && !gr.bh) || (pr.snr && !pr.bh)) return HS_ERR_INVALID_ARG;
     HsStats st_g, st_p;
     hs_status rc = HS_OK;
@@ -392,6 +394,22 @@ hs_status run_host(hs_plan_s* p, const float* hx, const float* hb, const HostFor
     return result;
 }
 
+template <int L>
+hs_status launch_presto_tile_2d(hs_plan_s* p, const HsStats& st, const HsIO& io, cudaStream_t stream) {
+    constexpr int W = 2;
+    constexpr int smem = 4 * hs_tile::smem_words(L, W);
+    static std::atomic<uint64_t> opted{0};
+    HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, false, true>, smem, p->device, opted));
+    constexpr int T = hs_tile::TILE * W;
+    const HsShape& sh = p->shape;
+    dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
+    hs_presto_tile_kernel<L, W, false, true><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+    p->last_kernel = "hs_presto_tile_kernel<W=2,2d>";
+    p->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
 bool presto_flags_ok(uint32_t flags) { return !((flags & HS_PRESTO_ALL_ORDERS) && !(flags & HS_PRESTO_ALL_HARMONICS)); }
 
 }  // namespace
@@ -427,11 +445,85 @@ hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
     p->shape.H = H;
     p->shape.flags = flags;
     p->tune = 0;
+    p->two_d = false;
+    p->shape.Z = 0;
     p->device = device;
     p->sm_count = sms;
     p->launches = 0;
     p->last_kernel = "";
     *plan = p;
+    return HS_OK;
+}
+
+hs_status hs_plan_2d(hs_plan_t* plan, int64_t n_bins, int32_t n_z, int32_t H, int64_t in_stride, int64_t out_stride,
+                     uint32_t flags, int32_t device) {
+    if (!plan) return HS_ERR_INVALID_ARG;
+    *plan = nullptr;
+    // k r and 2 k r + H' stay in 32 bits for k <= 16
+    if (n_bins < 2 || n_bins > (1ll << 25) || n_z < 1 || !(n_z & 1) || n_z > 65535 || H < 1 || H > 16) return HS_ERR_INVALID_ARG;
+    const hs_status rc = hs_plan(plan, n_bins, n_z, H, in_stride, out_stride, 0, flags, device);
+    if (rc != HS_OK) return rc;
+    (*plan)->two_d = true;
+    (*plan)->shape.Z = (n_z - 1) / 2;
+    return HS_OK;
+}
+
+hs_status hs_run_greedy_2d(hs_plan_t plan, const float* d_plane, const float* mu, const float* sigma,
+                           float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream) {
+    hs_status rc = check_device_args(plan, d_plane, nullptr, d_snr, d_best_h, d_path);
+    if (rc != HS_OK) return rc;
+    if (!plan->two_d) return HS_ERR_INVALID_ARG;
+    HsStats st;
+    rc = fill_stats(plan, mu, sigma, &st);
+    if (rc != HS_OK) return rc;
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    const HsShape& sh = plan->shape;
+    HsIO io{d_plane, nullptr, d_snr, d_best_h, d_path, nullptr, nullptr};
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    constexpr int BLOCK = 256, R = 2;
+    dim3 grid((unsigned)((sh.n_bins + BLOCK * R - 1) / (BLOCK * R)), (unsigned)sh.n_spectra);
+    const bool fs = !(sh.flags & HS_GREEDY_NO_FUND_SELECT), wp = d_path != nullptr, drift = !(sh.flags & HS_GREEDY_NO_DRIFT);
+    if (!drift) {
+        if (wp) hs_greedy2d_kernel<BLOCK, R, true, true, false><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+        else hs_greedy2d_kernel<BLOCK, R, true, false, false><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    } else if (fs && wp) hs_greedy2d_kernel<BLOCK, R, true, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else if (fs) hs_greedy2d_kernel<BLOCK, R, true, false, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else if (wp) hs_greedy2d_kernel<BLOCK, R, false, true, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    else hs_greedy2d_kernel<BLOCK, R, false, false, true><<<grid, BLOCK, 0, stream>>>(sh, st, io);
+    plan->last_kernel = "hs_greedy2d_kernel";
+    plan->launches += 1;
+    HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+hs_status hs_run_presto_2d(hs_plan_t plan, const float* d_plane, const float* mu, const float* sigma,
+                           float* d_snr, int32_t* d_best_h, void* cuda_stream) {
+    hs_status rc = check_device_args(plan, d_plane, nullptr, d_snr, d_best_h, nullptr);
+    if (rc != HS_OK) return rc;
+    if (!plan->two_d) return HS_ERR_INVALID_ARG;
+    HsStats st;
+    rc = fill_stats(plan, mu, sigma, &st);
+    if (rc != HS_OK) return rc;
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    const HsShape& sh = plan->shape;
+    HsIO io{d_plane, nullptr, d_snr, d_best_h, nullptr, nullptr, nullptr};
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (!(sh.flags & (HS_PRESTO_ALL_HARMONICS | HS_PRESTO_ALL_ORDERS)) && plan->tune != HS_TUNE_GENERIC) {
+        switch (floor_log2(sh.H)) {
+            case 0: return launch_presto_tile_2d<0>(plan, st, io, stream);
+            case 1: return launch_presto_tile_2d<1>(plan, st, io, stream);
+            case 2: return launch_presto_tile_2d<2>(plan, st, io, stream);
+            case 3: return launch_presto_tile_2d<3>(plan, st, io, stream);
+            default: return launch_presto_tile_2d<4>(plan, st, io, stream);
+        }
+    }
+    dim3 grid((unsigned)((sh.n_bins + 255) / 256), (unsigned)sh.n_spectra);
+    hs_presto2d_generic_kernel<<<grid, 256, 0, stream>>>(sh, st, io);
+    plan->last_kernel = "hs_presto2d_generic_kernel";
+    plan->launches += 1;
+    HS_CUDA(cudaGetLastError());
     return HS_OK;
 }
 
@@ -445,6 +537,7 @@ hs_status hs_run_greedy(hs_plan_t plan, const float* d_spectra, const float* d_i
                         const float* sigma, float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream) {
     hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, d_path);
     if (rc != HS_OK) return rc;
+    if (plan->two_d) return HS_ERR_INVALID_ARG;
     HsStats st;
     rc = fill_stats(plan, mu, sigma, &st);
     if (rc != HS_OK) return rc;
@@ -458,6 +551,7 @@ hs_status hs_run_presto(hs_plan_t plan, const float* d_spectra, const float* d_i
                         const float* sigma, float* d_snr, int32_t* d_best_h, void* cuda_stream) {
     hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, nullptr);
     if (rc != HS_OK) return rc;
+    if (plan->two_d) return HS_ERR_INVALID_ARG;
     HsStats st;
     rc = fill_stats(plan, mu, sigma, &st);
     if (rc != HS_OK) return rc;
@@ -471,7 +565,7 @@ hs_status hs_run_greedy_dstats(hs_plan_t plan, const float* d_spectra, const flo
                                const float* d_sigma, float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream) {
     hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, d_path);
     if (rc != HS_OK) return rc;
-    if (!d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
+    if (plan->two_d || !d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
     HsStats st;
     std::memset(&st, 0, sizeof(st));
     DeviceGuard guard(plan->device);
@@ -484,7 +578,7 @@ hs_status hs_run_presto_dstats(hs_plan_t plan, const float* d_spectra, const flo
                                const float* d_sigma, float* d_snr, int32_t* d_best_h, void* cuda_stream) {
     hs_status rc = check_device_args(plan, d_spectra, d_inv_baseline, d_snr, d_best_h, nullptr);
     if (rc != HS_OK) return rc;
-    if (!d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
+    if (plan->two_d || !d_mu || !d_sigma || (reinterpret_cast<uintptr_t>(d_mu) & 3u) || (reinterpret_cast<uintptr_t>(d_sigma) & 3u)) return HS_ERR_INVALID_ARG;
     HsStats st;
     std::memset(&st, 0, sizeof(st));
     DeviceGuard guard(plan->device);
@@ -501,7 +595,7 @@ int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip) {
 hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
                             int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
                             float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream) {
-    if (!plan || !d_spectra || !d_mu || !d_sigma || !d_work) return HS_ERR_INVALID_ARG;
+    if (!plan || plan->two_d || !d_spectra || !d_mu || !d_sigma || !d_work) return HS_ERR_INVALID_ARG;
     const HsShape& sh = plan->shape;
     if (n_hi == 0) n_hi = sh.n_bins;
     if (n_lo < 0 || n_hi > sh.n_bins || n_lo > n_hi || n_clip < 0 || n_clip > 16 || !(clip_sigma > 0.f)) return HS_ERR_INVALID_ARG;

@@ -23,6 +23,7 @@ struct HsShape {
     int n_spectra;         // S
     int H;                 // maximum harmonic order
     unsigned flags;        // HS_* algorithm flags (hs.h)
+    int Z;                 // 2-D plans (hs_plan_2d): rows are z = -Z .. Z, n_spectra = 2 Z + 1; 0 otherwise
 };
 
 struct HsIO {

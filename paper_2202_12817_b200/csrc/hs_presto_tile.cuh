@@ -124,7 +124,8 @@ struct Direct {
 };
 
 template <int L>
-__device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__ x, int N, int n, int i16, bool interior, bool al32) {
+__device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__ x, const float* __restrict__ x16, int N, int n, int i16,
+                                            bool interior, bool al32) {     // x16: the row fraction 16/32 reads from (x itself in 1-D)
     if (interior) {
         if (al32) {
             asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
@@ -138,15 +139,15 @@ __device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__
         }
         if (L >= 1) {
             asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];\n"
-                         : "=f"(d.yr[0]), "=f"(d.yr[1]), "=f"(d.yr[2]), "=f"(d.yr[3]) : "l"(x + i16));
-            asm volatile("ld.global.nc.f32 %0, [%1];\n" : "=f"(d.yr[4]) : "l"(x + i16 + 4));
+                         : "=f"(d.yr[0]), "=f"(d.yr[1]), "=f"(d.yr[2]), "=f"(d.yr[3]) : "l"(x16 + i16));
+            asm volatile("ld.global.nc.f32 %0, [%1];\n" : "=f"(d.yr[4]) : "l"(x16 + i16 + 4));
         }
     } else {                                                 // the last tile of a row: element-wise, zero beyond the end
 #pragma unroll
         for (int u = 0; u < 8; ++u) d.xr[u] = (n + u < N) ? __ldg(x + n + u) : 0.f;
         if (L >= 1) {
 #pragma unroll
-            for (int u = 0; u < 5; ++u) d.yr[u] = (i16 + u < N) ? __ldg(x + i16 + u) : 0.f;
+            for (int u = 0; u < 5; ++u) d.yr[u] = (i16 + u < N) ? __ldg(x16 + i16 + u) : 0.f;
         }
     }
 }
@@ -216,7 +217,10 @@ __device__ __forceinline__ void store8(float* __restrict__ ps, int* __restrict__
 }  // namespace hs_tile
 
 // grid: (tiles of 512 W outputs, spectra); block: 64 W threads; dynamic shared memory: 4 smem_words(L, W) bytes
-template <int L, int W, bool DSTATS = false>
+// TWOD (hs_plan_2d, reading R15): blockIdx.y is the row z + Z of an f-fdot plane and the term of fraction kk/32 is read
+// from row Round(kk z / 32) = (kk z + 16) >> 5 (arithmetic shift = floor: half up also for negative z) -- the same
+// for the whole tile, so every span is still one contiguous copy, only from its own row.
+template <int L, int W, bool DSTATS = false, bool TWOD = false>
 __global__ void __launch_bounds__(64 * W)
 hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     using namespace hs_tile;
@@ -231,7 +235,11 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int N = (int)sh.n_bins, n_fund = (int)sh.n_fund;
     const int n0 = blockIdx.x * (TILE * W);
     const int b0 = blockIdx.x * (TILE * W / 32);            // n0 / 32: the span of fraction kk starts at element kk b0
-    const float* x = io.x + (long long)s * sh.in_stride;
+    const float* x = io.x + (long long)s * sh.in_stride;                  // the row of x[n] itself (fraction 32/32)
+    const int zq = s - sh.Z;                                                 // TWOD: z of this row
+    auto frac_row = [&](int kk) -> const float* {                           // the row fraction kk/32 reads from
+        return TWOD ? io.x + (long long)(((kk * zq + 16) >> 5) + sh.Z) * sh.in_stride : x;
+    };
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (NF > 2) {
         if (threadIdx.x == 0) {
@@ -257,7 +265,7 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
                 const unsigned bytes = 4u * (unsigned)max(0ll, min((long long)span_words(kk, W), room));
                 if (bytes)
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                                 :: "r"(smem_u32(sm + span_off(f, W))), "l"(x + kk * b0), "r"(bytes), "r"(smem_u32(&bar)) : "memory");
+                                 :: "r"(smem_u32(sm + span_off(f, W))), "l"(frac_row(kk) + kk * b0), "r"(bytes), "r"(smem_u32(&bar)) : "memory");
             }
         }
     }
@@ -265,7 +273,7 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int w = warp >> 1, half = warp & 1;
     const int nw = n0 + TILE * w;
     Direct d;
-    load_direct<L>(d, x, N, nw + 16 * lane + 8 * half, nw / 2 + 8 * lane + 4 * half, nw + TILE + 8 <= N,
+    load_direct<L>(d, x, frac_row(16), N, nw + 16 * lane + 8 * half, nw / 2 + 8 * lane + 4 * half, nw + TILE + 8 <= N,
                    (reinterpret_cast<uintptr_t>(x) & 31u) == 0);
     if (NF > 2) mbar_wait(smem_u32(&bar), 0);
     float best[8];

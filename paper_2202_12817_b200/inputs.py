@@ -268,3 +268,72 @@ def delta_train(n_bins: int, f0: int, K: int, A: float) -> torch.Tensor:
     for k in range(1, K + 1):
         x[k * f0] = A
     return x
+
+
+# ----------------------------------------------------------------------------------------------
+# configs[4] (NEXT-4): an f-fdot plane -- n_z = 2 Z + 1 rows (z = -Z .. Z) of n_bins Exp(1) powers with drifting signals
+# ----------------------------------------------------------------------------------------------
+@dataclass
+class Drifter:
+    r: float          # fractional fundamental frequency bin
+    z: float          # fractional fundamental drift (f-dot) row
+    duty: float
+    amp: float
+    phase: float
+
+
+@dataclass
+class PlaneWorkload:
+    name: str
+    n_z: int
+    n_bins: int
+    H: int
+    seed: int
+    n_signals: int
+    signals: List[Drifter] = field(default_factory=list)
+
+    def __post_init__(self):
+        Z = (self.n_z - 1) // 2
+        zmax = max(0.0, Z / 16.0 - 0.25)                 # all 16 harmonics of every signal stay inside the plane
+        self.signals = []
+        for j in range(self.n_signals):
+            u = [hash_u01(self.seed, 0xD51F, j, q) for q in range(5)]
+            self.signals.append(Drifter(r=100.0 + u[0] * (self.n_bins / 16.0 - 100.0), z=(2.0 * u[1] - 1.0) * zmax,
+                                        duty=0.02 + u[2] * 0.18, amp=6.0 + u[3] * 8.0, phase=2.0 * math.pi * u[4]))
+
+
+def plane_workload(name: str) -> PlaneWorkload:
+    if name == "cfg5":      # BASELINE.json configs[4]: 2^21 frequency bins x 201 fdot rows, 32 drifting signals, H = 16
+        return PlaneWorkload("cfg5", 201, 1 << 21, 16, seed=5, n_signals=32)
+    raise KeyError(name)
+
+
+def generate_plane(w: PlaneWorkload, device="cpu", n_bins: Optional[int] = None) -> torch.Tensor:
+    """[n_z, N] fp32 plane: |complex Gaussian noise + signals|^2.  Harmonic k of a signal sits at (k r, k z): the DFT
+    response in r (as in the 1-D generator) is put into the row floor(k z) with weight cos^2 and the row above with
+    weight sin^2 of the fractional part (a stand-in for the f-dot response; none of the method's arithmetic)."""
+    n = w.n_bins if n_bins is None else n_bins
+    Z = (w.n_z - 1) // 2
+    out = torch.empty((w.n_z, n), dtype=torch.float32, device=device)
+    for zi in range(w.n_z):
+        re, im = noise_row_complex(w.seed, zi, n, device)
+        for sg in w.signals:
+            for k in range(1, 17):
+                zz = k * sg.z
+                row = math.floor(zz)
+                frac = zz - row
+                for rr, wgt in ((row, math.cos(0.5 * math.pi * frac) ** 2), (row + 1, math.sin(0.5 * math.pi * frac) ** 2)):
+                    if rr + Z != zi or wgt < 1e-6 or k * sg.r >= n - 1:
+                        continue
+                    g = math.exp(-((math.pi * sg.duty * k) ** 2) / (4.0 * math.log(2.0)))
+                    g1 = math.exp(-((math.pi * sg.duty) ** 2) / (4.0 * math.log(2.0)))
+                    amp = sg.amp * g / g1 * math.sqrt(wgt)
+                    pos = k * sg.r
+                    b = torch.arange(max(0, math.floor(pos) - 8), min(n, math.floor(pos) + 10), device=device)
+                    dlt = b.to(torch.float64) - pos
+                    resp = amp * torch.sinc(dlt)
+                    ang = sg.phase * k - math.pi * dlt
+                    re[b] += (resp * torch.cos(ang)).to(re.dtype)
+                    im[b] += (resp * torch.sin(ang)).to(im.dtype)
+        out[zi].copy_((re * re + im * im).to(torch.float32))
+    return out

@@ -20,7 +20,7 @@ def lib():
 def _declared_symbols():
     src = open(os.path.join(ROOT, "include", "hs.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(hs_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(hs_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_symbols_exported(lib):

@@ -1,5 +1,7 @@
 """GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle on
 the same seeded inputs.  Acceptance rules in tests/parity.py."""
+import math
+
 import numpy as np
 import pytest
 import torch
@@ -740,3 +742,148 @@ def test_dstats_equals_by_value_statistics(hs, oracle_mod):
             assert torch.equal(out[0][:, :N].view(torch.int32), out[2][:, :N].view(torch.int32)) and torch.equal(out[1][:, :N], out[3][:, :N])
     finally:
         hs.hs_destroy(plan)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-4 (reading R15): 2-D harmonic sums over an f-fdot plane
+# ------------------------------------------------------------------------------------------
+def _run_2d(hs, P, H, mu, sg, flags, form, tune=0, want_path=True):
+    P = torch.as_tensor(P)
+    nz, N = P.shape
+    istr = (N + 3) & ~3
+    dP = torch.zeros((nz, istr), dtype=torch.float32, device="cuda")
+    dP[:, :N] = P.cuda()
+    snr = torch.full((nz, istr), float("nan"), dtype=torch.float32, device="cuda")
+    bh = torch.full((nz, istr), -7, dtype=torch.int32, device="cuda")
+    path = torch.full((nz, istr), -7, dtype=torch.int32, device="cuda") if (want_path and form == "greedy") else None
+    plan = hs.hs_plan_2d(N, nz, H, istr, istr, flags, 0)
+    try:
+        hs.hs_plan_set_tuning(plan, tune)
+        if form == "greedy":
+            hs.hs_run_greedy_2d(plan, dP, mu, sg, snr, bh, path)
+        else:
+            hs.hs_run_presto_2d(plan, dP, mu, sg, snr, bh)
+        torch.cuda.synchronize()
+        kern = hs.hs_last_kernel(plan)
+    finally:
+        hs.hs_destroy(plan)
+    assert torch.all(torch.isnan(snr[:, N:])) and torch.all(bh[:, N:] == -7)
+    return snr[:, :N].cpu().numpy(), bh[:, :N].cpu().numpy(), (path[:, :N].cpu().numpy() if path is not None else None), kern
+
+
+PLANES = [(1, 2), (1, 700), (3, 3), (5, 4099), (41, 1000), (201, 3001), (9, 70001)]
+
+
+@pytest.mark.parametrize("H", [1, 2, 5, 8, 16])
+def test_2d_exact_integer(hs, oracle_mod, H):
+    """Exact-integer planes, ragged shapes: greedy 2-D (ours) / simple 2-D / PRESTO-like 2-D family against the oracle
+    bit for bit (snr, best_h, path), tile kernel and coverage kernel."""
+    mu, sg = _int_stats(H)
+    for nz, N in PLANES:
+        P = inputs.integer_spectra(500 + N + nz, nz, N, 255).numpy()
+        for flags in (0, NO_FUND_SELECT, NO_DRIFT):
+            s_ref, b_ref, p_ref = oracle_mod.greedy_2d(P, H, mu, sg, flags)
+            s, b, p, _ = _run_2d(hs, P, H, mu, sg, flags, "greedy")
+            assert np.array_equal(p.view(np.uint32), p_ref), (nz, N, flags)
+            assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref), (nz, N, flags)
+        for flags, tunes in ((0, (0, GENERIC)), (ALL_HARMONICS, (0,)), (ALL_HARMONICS | ALL_ORDERS, (0,))):
+            s_ref, b_ref = oracle_mod.presto_2d(P, H, mu, sg, flags)
+            for tune in tunes:
+                s, b, _, kern = _run_2d(hs, P, H, mu, sg, flags, "presto", tune=tune)
+                assert kern.startswith("hs_presto_tile_kernel" if (flags == 0 and tune == 0) else "hs_presto2d_generic_kernel")
+                assert np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref), (nz, N, flags, tune)
+
+
+def _check_2d(snr_ref, bh_ref, snr, bh, mu, sg, T=10.0):
+    """tests/parity.py rules for a plane; where best_h differs the two maxima must agree within the near-tie tolerance."""
+    from parity import REL, _tol
+    mu = np.asarray(mu, np.float64); sg = np.asarray(sg, np.float64)
+    snr = snr.astype(np.float64)
+    tol = _tol(snr_ref, mu, sg)
+    S = snr_ref * sg[bh_ref - 1] + mu[bh_ref - 1]
+    bound = np.where(snr_ref >= 1.0, REL * np.abs(snr_ref), REL * (np.abs(S) + mu[bh_ref - 1]) / sg[bh_ref - 1])
+    err = np.abs(snr - snr_ref)
+    assert np.all(err <= bound), err.max()
+    bad = bh != bh_ref
+    assert np.all(err[bad] <= tol[bad])
+    near = np.abs(snr_ref - T) <= tol
+    assert np.array_equal((snr >= T) & ~near, (snr_ref >= T) & ~near)
+    return int(bad.sum())
+
+
+def test_2d_cfg5_content_reduced(hs, oracle_mod):
+    """configs[4] content (Exp(1) plane with drifting signals) at 41 x 2^16, H = 16: all three forms within the
+    tolerances of tests/parity.py; the greedy path is bit-exact; every injected signal is a candidate of the greedy form."""
+    H = 16
+    w = inputs.PlaneWorkload("p", 41, 1 << 16, H, seed=5, n_signals=4)
+    P = inputs.generate_plane(w, "cuda").cpu().numpy()
+    Z = 20
+    for flags, variant in ((0, "greedy"), (NO_DRIFT, "simple")):
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("simple", H))      # any statistics do: parity does not depend on them
+        s_ref, b_ref, p_ref = oracle_mod.greedy_2d(P, H, mu, sg, flags)
+        s, b, p, _ = _run_2d(hs, P, H, mu, sg, flags, "greedy")
+        assert np.array_equal(p.view(np.uint32), p_ref)
+        _check_2d(s_ref, b_ref, s, b, mu, sg)
+        if flags == 0:
+            for sgn in w.signals:
+                r0, z0 = int(math.floor(sgn.r)), int(math.floor(sgn.z))
+                assert s[z0 + Z - 1:z0 + Z + 2, r0 - 1:r0 + 2].max() > 10.0
+    for flags, variant in ((0, "presto"), (ALL_HARMONICS, "presto_all")):
+        mu, sg = (t.numpy() for t in inputs.exp1_stats(variant, H))
+        s_ref, b_ref = oracle_mod.presto_2d(P, H, mu, sg, flags)
+        s, b, _, _ = _run_2d(hs, P, H, mu, sg, flags, "presto")
+        _check_2d(s_ref, b_ref, s, b, mu, sg)
+
+
+def test_2d_cfg5_full_size_sampled_rows(hs, oracle_mod):
+    """configs[4] at its real size (201 x 2^21, H = 16) through one call per form, as bench.py --workload cfg5 times it;
+    rows z = -100, -6, -1, 0, 1, 3, 50, 100 against the oracle (which reads the whole plane but computes those rows)."""
+    w = inputs.plane_workload("cfg5")
+    H, nz, N = w.H, w.n_z, w.n_bins
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12 * (1 << 30):
+        pytest.skip("needs 12 GiB of device memory")
+    dP = inputs.generate_plane(w, "cuda")
+    P = dP.cpu().numpy()
+    snr = torch.empty((nz, N), dtype=torch.float32, device="cuda")
+    bh = torch.empty((nz, N), dtype=torch.int32, device="cuda")
+    path = torch.empty((nz, N), dtype=torch.int32, device="cuda")
+    rows = [0, 94, 99, 100, 101, 103, 150, 200]
+    plan = hs.hs_plan_2d(N, nz, H)
+    try:
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("simple", H))
+        hs.hs_run_greedy_2d(plan, dP, mu, sg, snr, bh, path)
+        torch.cuda.synchronize()
+        assert int(bh.min()) >= 1 and int(bh.max()) <= H and bool(torch.isfinite(snr).all())
+        for zi in rows:
+            s_ref, b_ref, p_ref = oracle_mod.greedy_2d(P, H, mu, sg, 0, rows=(zi, zi + 1))
+            assert np.array_equal(path[zi].cpu().numpy().view(np.uint32), p_ref[zi])
+            _check_2d(s_ref[zi:zi + 1], b_ref[zi:zi + 1], snr[zi:zi + 1].cpu().numpy(), bh[zi:zi + 1].cpu().numpy(), mu, sg)
+        mu, sg = (t.numpy() for t in inputs.exp1_stats("presto", H))
+        hs.hs_run_presto_2d(plan, dP, mu, sg, snr, bh)
+        torch.cuda.synchronize()
+        assert hs.hs_last_kernel(plan).startswith("hs_presto_tile_kernel")
+        assert int(bh.min()) >= 1 and int(bh.max()) <= H and bool(torch.isfinite(snr).all())
+        for zi in rows:
+            s_ref, b_ref = oracle_mod.presto_2d(P, H, mu, sg, 0, rows=(zi, zi + 1))
+            _check_2d(s_ref[zi:zi + 1], b_ref[zi:zi + 1], snr[zi:zi + 1].cpu().numpy(), bh[zi:zi + 1].cpu().numpy(), mu, sg)
+    finally:
+        hs.hs_destroy(plan)
+
+
+def test_2d_plans_and_1d_entry_points_do_not_mix(hs):
+    mu, sg = _int_stats(8)
+    x = torch.ones((3, 1024), device="cuda"); snr = torch.empty_like(x); bh = torch.empty((3, 1024), dtype=torch.int32, device="cuda")
+    p2 = hs.hs_plan_2d(1024, 3, 8)
+    p1 = hs.hs_plan(1024, 3, 8)
+    try:
+        with pytest.raises(hs.HsError):
+            hs.hs_run_greedy(p2, x, None, mu, sg, snr, bh)
+        with pytest.raises(hs.HsError):
+            hs.hs_run_presto_2d(p1, x, mu, sg, snr, bh)
+        with pytest.raises(hs.HsError):
+            hs.hs_plan_2d(1024, 4, 8)            # n_z must be odd
+        with pytest.raises(hs.HsError):
+            hs.hs_plan_2d(1024, 3, 32)           # H <= 16
+    finally:
+        hs.hs_destroy(p1); hs.hs_destroy(p2)
