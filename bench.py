@@ -425,8 +425,12 @@ def run_cuda(args):
         if rec is None or not l2 or not rec.get("l2_to_sm_sector_bytes"):
             return None
         floor_ms = rec["l2_to_sm_sector_bytes"] / (l2 * 1e9) * 1e3
-        return {"l2_to_sm_gbs": l2, "sector_bytes_per_launch": rec["l2_to_sm_sector_bytes"],
-                "ceiling_ms": floor_ms, "frac_of_ceiling": floor_ms / ms, "source": mm.get("source"), "capture": rec.get("capture")}
+        out = {"l2_to_sm_gbs": l2, "sector_bytes_per_launch": rec["l2_to_sm_sector_bytes"],
+               "ceiling_ms": floor_ms, "frac_of_ceiling": floor_ms / ms, "source": mm.get("source"), "capture": rec.get("capture")}
+        if rec.get("access_form_ceiling_ms"):      # the measured rate of the kernel's own access form (L1 line requests included)
+            out.update(access_form_ceiling_ms=rec["access_form_ceiling_ms"], frac_of_access_form_ceiling=rec["access_form_ceiling_ms"] / ms,
+                       access_form_note=rec.get("access_form_note"))
+        return out
 
     def per_kernel(form, ms):
         rec = evidence(form)
