@@ -68,6 +68,9 @@ def parse_args():
     ap.add_argument("--stats", default="auto", choices=["auto", "given", "estimated"],
                     help="given: closed-form Exp(1) statistics passed by value; estimated: hs_estimate_stats (reading R14 of "
                          "GetMeanStdev) inside the step, then hs_run_*_dstats; auto = estimated for the red-noise workload (cfg4)")
+    ap.add_argument("--whiten", default="pass", choices=["pass", "fused"],
+                    help="red-noise workload (cfg4): pass = hs_whiten writes x * inv_baseline once and the sums read that array; "
+                         "fused = every gather multiplies (two arrays read by the gather)")
     ap.add_argument("--tune-greedy", type=int, default=0)
     ap.add_argument("--tune-presto", type=int, default=0)
     return ap.parse_args()
@@ -279,34 +282,44 @@ def run_cuda(args):
         dmu_p = torch.empty_like(dmu_g); dsg_p = torch.empty_like(dmu_g)
         work = torch.empty(hs.hs_stats_workspace_bytes(plan_g, n_clip) // 8, dtype=torch.float64, device=dev)
 
+    # the whitening pass writes y = x * inv_baseline once; the sums then read y alone (same bits, reading R13)
+    wpass = ib is not None and args.whiten == "pass"
+    y = torch.empty_like(x) if wpass else None
+
     def step(ev=None):
         if ev is not None:
             ev[0].record(stream)
+        xin, bin_ = x, ib
+        if wpass:
+            hs.hs_whiten(plan_g, x, ib, y, stream.cuda_stream)
+            xin, bin_ = y, None
+        if ev is not None:
+            ev[4].record(stream)
         if est:
             if do_g:
-                hs.hs_estimate_stats(plan_g, True, x, ib, N // 64, N // 32, clip, n_clip, dmu_g, dsg_g, work, stream.cuda_stream)
+                hs.hs_estimate_stats(plan_g, True, xin, bin_, N // 64, N // 32, clip, n_clip, dmu_g, dsg_g, work, stream.cuda_stream)
             if do_p:
-                hs.hs_estimate_stats(plan_p, False, x, ib, N // 64, N // 32, clip, n_clip, dmu_p, dsg_p, work, stream.cuda_stream)
+                hs.hs_estimate_stats(plan_p, False, xin, bin_, N // 64, N // 32, clip, n_clip, dmu_p, dsg_p, work, stream.cuda_stream)
         if ev is not None:
             ev[3].record(stream)
         if do_g:
             if est:
-                hs.hs_run_greedy_dstats(plan_g, x, ib, dmu_g, dsg_g, snr_g, bh_g, None, stream.cuda_stream)
+                hs.hs_run_greedy_dstats(plan_g, xin, bin_, dmu_g, dsg_g, snr_g, bh_g, None, stream.cuda_stream)
             else:
-                hs.hs_run_greedy(plan_g, x, ib, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
+                hs.hs_run_greedy(plan_g, xin, bin_, mu_g, sg_g, snr_g, bh_g, None, stream.cuda_stream)
         if ev is not None:
             ev[1].record(stream)
         if do_p:
             if est:
-                hs.hs_run_presto_dstats(plan_p, x, ib, dmu_p, dsg_p, snr_p, bh_p, stream.cuda_stream)
+                hs.hs_run_presto_dstats(plan_p, xin, bin_, dmu_p, dsg_p, snr_p, bh_p, stream.cuda_stream)
             else:
-                hs.hs_run_presto(plan_p, x, ib, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
+                hs.hs_run_presto(plan_p, xin, bin_, mu_p, sg_p, snr_p, bh_p, stream.cuda_stream)
         if ev is not None:
             ev[2].record(stream)
 
     for _ in range(args.warmup):
         step()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -319,7 +332,8 @@ def run_cuda(args):
     launches = hs.hs_launch_count(plan_g) + hs.hs_launch_count(plan_p) - l0
     kname = {"greedy": hs.hs_last_kernel(plan_g) if do_g else None, "presto": hs.hs_last_kernel(plan_p) if do_p else None}
     total_ms = evs[0][0].elapsed_time(evs[-1][2])          # device time of exactly K steps
-    s_ms = sum(e[0].elapsed_time(e[3]) for e in evs) / args.steps
+    w_ms = sum(e[0].elapsed_time(e[4]) for e in evs) / args.steps
+    s_ms = sum(e[4].elapsed_time(e[3]) for e in evs) / args.steps
     g_ms = sum(e[3].elapsed_time(e[1]) for e in evs) / args.steps
     p_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
     # clocks: keep the sampler running through a few more device-only steps so short runs still get samples
@@ -335,6 +349,10 @@ def run_cuda(args):
     g_ms = max_over_ranks(g_ms, dev)
     p_ms = max_over_ranks(p_ms, dev)
     s_ms = max_over_ranks(s_ms, dev)
+    w_ms = max_over_ranks(w_ms, dev)
+    if wpass:                       # the whitening pass belongs to each form's 16 B/bin (x and the multiplier read once)
+        g_ms += w_ms if do_g else 0.0
+        p_ms += w_ms if (do_p and not do_g) else 0.0
     bins_step = float(S) * N * world
     n_forms = int(do_g) + int(do_p)
     default_run = (args.forms == "both" and not args.greedy_flags and not args.presto_flags and ib is None
@@ -471,6 +489,7 @@ def run_cuda(args):
                                        (", per-bin inverse baseline" if ib is not None else ""),
                            "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
+                "whiten": ({"source": "hs_whiten pass inside the step; its time is counted in the form's launch_ms (16 B/bin)", "ms": w_ms} if wpass else None),
                 "stats": ({"source": "hs_estimate_stats inside the step (reading R14): bins [N/64, N/32), 2 rejection rounds at 3 sigma, "
                                      "then hs_run_*_dstats", "ms": s_ms} if est else
                           {"source": "closed-form Exp(1) statistics passed by value", "ms": 0.0}),

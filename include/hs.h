@@ -140,6 +140,13 @@ hs_status hs_run_presto_dstats(hs_plan_t plan, const float* d_spectra, const flo
                                const float* d_mu, const float* d_sigma,
                                float* d_snr, int32_t* d_best_h, void* cuda_stream);
 
+/* Spectrum whitening as a pass of its own: d_whitened[s][b] = d_spectra[s][b] * d_inv_baseline[s][b]
+ * for b < n_bins, ONE fp32 multiply -- the product the fused path forms (reading R13) -- so that
+ * hs_run_*(plan, d_whitened, NULL, ..) returns the bits of hs_run_*(plan, d_spectra, d_inv_baseline, ..) while its
+ * gather reads one array instead of two (cfg4: 4.0 + 11.6 ms instead of 26 ms).  d_whitened: device, [S][in_stride],
+ * 16-byte aligned, not aliasing the inputs; elements beyond n_bins of a row are not written.  Asynchronous. */
+hs_status hs_whiten(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline, float* d_whitened, void* cuda_stream);
+
 /* The step before the path: "{mu, sigma} = GetMeanStdev()", "the mean and standard deviation ...
  * for partial sum of length H", the pre-processing all algorithms share.  The paper does
  * not define it; reading R14 of DESIGN.md: for every spectrum s and order h, the mean and the population standard

@@ -26,7 +26,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
-           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes",
+           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes", "hs_whiten",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -81,6 +81,8 @@ def load() -> ctypes.CDLL:
     lib.hs_run_presto_dstats.restype = ctypes.c_int
     lib.hs_estimate_stats.argtypes = [vp, i32, vp, vp, i64, i64, ctypes.c_float, i32, vp, vp, vp, i64, vp]
     lib.hs_estimate_stats.restype = ctypes.c_int
+    lib.hs_whiten.argtypes = [vp, vp, vp, vp, vp]
+    lib.hs_whiten.restype = ctypes.c_int
     lib.hs_stats_workspace_bytes.argtypes = [vp, i32]
     lib.hs_stats_workspace_bytes.restype = i64
     lib.hs_launch_count.argtypes = [vp]
@@ -208,6 +210,14 @@ def hs_run_presto_dstats(plan, d_spectra: torch.Tensor, d_inv_baseline: Optional
                                     _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"),
                                     _dptr(d_snr, torch.float32, "d_snr"), _dptr(d_best_h, torch.int32, "d_best_h"),
                                     stream), "hs_run_presto_dstats")
+
+
+def hs_whiten(plan, d_spectra: torch.Tensor, d_inv_baseline: torch.Tensor, d_whitened: torch.Tensor, stream: Optional[int] = None) -> None:
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_whiten(plan, _dptr(d_spectra, torch.float32, "d_spectra"), _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"),
+                         _dptr(d_whitened, torch.float32, "d_whitened"), stream), "hs_whiten")
 
 
 def hs_stats_workspace_bytes(plan, n_clip: int) -> int:

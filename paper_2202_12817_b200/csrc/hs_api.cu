@@ -587,6 +587,27 @@ hs_status hs_run_presto_dstats(hs_plan_t plan, const float* d_spectra, const flo
     return launch_presto(plan, plan->shape, st, io, (cudaStream_t)cuda_stream);
 }
 
+hs_status hs_whiten(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline, float* d_whitened, void* cuda_stream) {
+    if (!plan || plan->two_d || !d_spectra || !d_inv_baseline || !d_whitened) return HS_ERR_INVALID_ARG;
+    if (!aligned16(d_spectra) || !aligned16(d_inv_baseline) || !aligned16(d_whitened)) return HS_ERR_INVALID_ARG;
+    if ((const void*)d_whitened == (const void*)d_spectra || (const void*)d_whitened == (const void*)d_inv_baseline) return HS_ERR_INVALID_ARG;
+    const HsShape& sh = plan->shape;
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    for (long long s0 = 0; s0 < sh.n_spectra; s0 += HS_MAX_GRID_Y) {
+        const int rows = (int)std::min<long long>(HS_MAX_GRID_Y, sh.n_spectra - s0);
+        const long long n4 = std::max<long long>(1, sh.n_bins / 4);
+        const long long per_row = std::max(1ll, std::min((n4 + 255) / 256, (long long)std::max(1, plan->sm_count * 32 / rows + 1)));
+        dim3 grid((unsigned)per_row, (unsigned)rows);
+        hs_whiten_kernel<<<grid, 256, 0, stream>>>(d_spectra + s0 * sh.in_stride, d_inv_baseline + s0 * sh.in_stride,
+                                                   d_whitened + s0 * sh.in_stride, sh.in_stride, sh.in_stride, (int)sh.n_bins);
+        plan->launches += 1;
+        HS_CUDA(cudaGetLastError());
+    }
+    return HS_OK;
+}
+
 int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip) {
     if (!plan || n_clip < 0 || n_clip > 16) return -1;
     return (int64_t)(n_clip + 1) * plan->shape.n_spectra * HS_MAX_H * 3 * (int64_t)sizeof(double);
@@ -621,7 +642,8 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
                 HsIO io{d_spectra + s0 * sh.in_stride, d_inv_baseline ? d_inv_baseline + s0 * sh.in_stride : nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
                 HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, r ? acc + (r - 1) * per_round + s0 * HS_MAX_H * 3 : nullptr,
                               acc + r * per_round + s0 * HS_MAX_H * 3};
-                dim3 grid((unsigned)((count + 255) / 256), (unsigned)sub.n_spectra);
+                                const long long want = std::max(1ll, (count + 256 * 2 - 1) / (256 * 2));      // two groups of 32 bins per warp
+                dim3 grid((unsigned)want, (unsigned)sub.n_spectra);
                 if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (greedy) hs_stats_pass_kernel<true, false><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (d_inv_baseline) hs_stats_pass_kernel<false, true><<<grid, 256, 0, stream>>>(sub, io, a);

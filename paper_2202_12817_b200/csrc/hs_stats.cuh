@@ -6,11 +6,11 @@
 // edge, reading R4) do not count -- followed by n_clip rounds of outlier rejection: round p keeps the sums with
 // lo <= S_h(n) <= hi, lo / hi = mean -/+ clip * std of round p - 1, rounded to fp32.
 //
-// One launch per round: a thread owns one bin n and walks its orders exactly as the coverage kernels do (fp32 sums in
-// the written order), the kept sums of a warp are reduced by shuffles in fp64 (count, sum, sum of squares), added to
-// the CTA's accumulators in shared memory and from there to the round's accumulators in global memory (fp64 atomics:
-// the order of the additions is not fixed, the values agree to rounding).  A last tiny launch turns the accumulators
-// of the final round into mu / sigma.
+// One launch per round: a lane owns one bin n at a time and walks its orders exactly as the coverage kernels do (fp32
+// sums in the written order); the sums of a warp are transposed through shared memory so that lane h - 1 adds up order
+// h in fp64 (count, sum, sum of squares) in registers, and adds its totals to the round's accumulators in global
+// memory with fp64 atomics at the end (the order of the additions is not fixed, the values agree to rounding).  A last
+// tiny launch turns the accumulators of the final round into mu / sigma.
 #pragma once
 #include "hs_common.cuh"
 #include "hs_generic.cuh"
@@ -21,12 +21,6 @@ struct HsStatsArgs {
     const double* prev;            // accumulators of the round before ([S][32][3]: count, sum, sum of squares) or null
     double* acc;                   // accumulators of this round ([S][32][3]), zeroed by the caller
 };
-
-__device__ __forceinline__ double hs_warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    return v;
-}
 
 // mean and population standard deviation from (count, sum, sum of squares); no fused multiply-add, so that the
 // fp32 limits derived from them are those of a plain double-precision evaluation
@@ -39,91 +33,102 @@ __device__ __forceinline__ void hs_moments(const double* a, double& mean, double
     }
 }
 
+// grid: (chunks, spectra); a warp takes groups of 32 consecutive bins of [n_lo, n_hi) in a grid-stride loop.  Lane l walks
+// the orders of its bin and leaves S_h (NaN: order not evaluated, or rejected) in the warp's [order][lane] tile of
+// shared memory; then lane h - 1 adds up the 32 entries of order h in fp64 (count, sum, sum of squares) into its own
+// registers -- a transposition instead of 20 shuffles per order -- and adds them to global memory once, at the end.
 template <bool GREEDY, bool HAS_BASE>
 __global__ void __launch_bounds__(256)
 hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a) {
-    __shared__ double s_acc[HS_MAX_H][3];
-    __shared__ float s_lo[HS_MAX_H], s_hi[HS_MAX_H];
+    constexpr int WARPS = 8, PITCH = 33;                    // 33: both the lane-major stores and the order-major loads are conflict-free
+    __shared__ float s_v[WARPS][HS_MAX_H * PITCH];
     const int s = blockIdx.y;
-    if (threadIdx.x < HS_MAX_H) {
-        float lo = HS_NEG_INF, hi = -HS_NEG_INF;
-        if (a.prev) {
-            double mean, sd;
-            hs_moments(a.prev + ((long long)s * HS_MAX_H + threadIdx.x) * 3, mean, sd);
-            lo = __double2float_rn(__dsub_rn(mean, __dmul_rn(a.clip, sd)));
-            hi = __double2float_rn(__dadd_rn(mean, __dmul_rn(a.clip, sd)));
-        }
-        s_lo[threadIdx.x] = lo; s_hi[threadIdx.x] = hi;
-        s_acc[threadIdx.x][0] = 0.0; s_acc[threadIdx.x][1] = 0.0; s_acc[threadIdx.x][2] = 0.0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // rejection limits of this lane's order (lane = h - 1) from the accumulators of the round before
+    float lo = HS_NEG_INF, hi = -HS_NEG_INF;
+    if (a.prev) {
+        double mean, sd;
+        hs_moments(a.prev + ((long long)s * HS_MAX_H + lane) * 3, mean, sd);
+        lo = __double2float_rn(__dsub_rn(mean, __dmul_rn(a.clip, sd)));
+        hi = __double2float_rn(__dadd_rn(mean, __dmul_rn(a.clip, sd)));
     }
-    __syncthreads();
-    const long long n = a.n_lo + (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool have = n < a.n_hi;
     const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
     const float* __restrict__ ib = HAS_BASE ? io.inv_base + (long long)s * sh.in_stride : nullptr;
-    const int lane = threadIdx.x & 31;
+    float* tile = s_v[warp];
+    const float NOT = __int_as_float(0x7fc00000);           // NaN marks "no sample"
+    double cnt = 0.0, s1 = 0.0, s2 = 0.0;                   // of order lane + 1
 
-    auto add = [&](int h, bool valid, float v) {            // every lane of the warp calls this for every order
-        const bool keep = valid && v >= s_lo[h - 1] && v <= s_hi[h - 1];
-        const unsigned m = __ballot_sync(0xffffffffu, keep);
-        if (m == 0) return;
-        const double dv = keep ? (double)v : 0.0;
-        const double s1 = hs_warp_sum(dv), s2 = hs_warp_sum(__dmul_rn(dv, dv));
-        if (lane == 0) {
-            atomicAdd(&s_acc[h - 1][0], (double)__popc(m));
-            atomicAdd(&s_acc[h - 1][1], s1);
-            atomicAdd(&s_acc[h - 1][2], s2);
-        }
-    };
-
-    if (GREEDY) {                                           // Alg. 2 as hs_greedy_generic_kernel walks it
-        const long long last = sh.n_bins - 1;
-        const bool no_fs = sh.flags & HSF_NO_FUND_SELECT, no_drift = sh.flags & HSF_NO_DRIFT;
-        long long d = 0;
-        float sum = 0.f;
-        bool alive = have;
-        for (int h = 1; h <= sh.H; ++h) {
-            const long long m = (long long)h * n + d;
-            alive = alive && m <= last;
-            if (alive) {
-                const float av = hs_load<HAS_BASE>(x, ib, m);
-                float bv = HS_NEG_INF;
-                if (m + 1 <= last && !no_drift && !(h == 1 && no_fs)) bv = hs_load<HAS_BASE>(x, ib, m + 1);
-                const bool shift = bv > av;
-                d += shift;
-                sum = __fadd_rn(sum, shift ? bv : av);
-            }
-            add(h, alive, sum);
-        }
-    } else {                                                // Alg. 1 family as hs_presto_generic_kernel walks it
-        const bool all_h = sh.flags & HSF_ALL_HARMONICS, all_o = sh.flags & HSF_ALL_ORDERS;
-        for (int Hp = 1; Hp <= sh.H; Hp = all_o ? Hp + 1 : Hp * 2) {
+    const long long groups = (a.n_hi - a.n_lo + 31) / 32;
+    for (long long g = (long long)blockIdx.x * WARPS + warp; g < groups; g += (long long)gridDim.x * WARPS) {
+        const long long n = a.n_lo + g * 32 + lane;
+        const bool have = n < a.n_hi;
+#pragma unroll 1
+        for (int h = sh.H; h < HS_MAX_H; ++h) tile[h * PITCH + lane] = NOT;
+        if (GREEDY) {                                       // Alg. 2 as hs_greedy_generic_kernel walks it
+            const long long last = sh.n_bins - 1;
+            const bool no_fs = sh.flags & HSF_NO_FUND_SELECT, no_drift = sh.flags & HSF_NO_DRIFT;
+            long long d = 0;
             float sum = 0.f;
-            if (have) {
-                const unsigned den = 2u * Hp;
-                const unsigned qn = (unsigned)n / (unsigned)Hp, rn = 2u * ((unsigned)n - qn * Hp);
-                unsigned q = qn, r = rn + Hp;
-                if (r >= den) { r -= den; ++q; }
-                sum = hs_load<HAS_BASE>(x, ib, q);
-                const int step = all_h ? 1 : 2;
-                q += qn; r += rn;
-                if (r >= den) { r -= den; ++q; }
-                for (int h = 2; h <= Hp; h += step) {
-                    sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, q));
-                    for (int k = 0; k < step; ++k) {
-                        q += qn; r += rn;
-                        if (r >= den) { r -= den; ++q; }
+            bool alive = have;
+            for (int h = 1; h <= sh.H; ++h) {
+                const long long m = (long long)h * n + d;
+                alive = alive && m <= last;
+                if (alive) {
+                    const float av = hs_load<HAS_BASE>(x, ib, m);
+                    float bv = HS_NEG_INF;
+                    if (m + 1 <= last && !no_drift && !(h == 1 && no_fs)) bv = hs_load<HAS_BASE>(x, ib, m + 1);
+                    const bool shift = bv > av;
+                    d += shift;
+                    sum = __fadd_rn(sum, shift ? bv : av);
+                }
+                tile[(h - 1) * PITCH + lane] = alive ? sum : NOT;
+            }
+        } else {                                            // Alg. 1 family as hs_presto_generic_kernel walks it
+            const bool all_h = sh.flags & HSF_ALL_HARMONICS, all_o = sh.flags & HSF_ALL_ORDERS;
+            for (int Hp = 1; Hp <= sh.H; ++Hp) {
+                const bool in_set = all_o || (Hp & (Hp - 1)) == 0;
+                float sum = 0.f;
+                if (have && in_set) {
+                    const unsigned den = 2u * Hp;
+                    const unsigned qn = (unsigned)n / (unsigned)Hp, rn = 2u * ((unsigned)n - qn * Hp);
+                    unsigned q = qn, r = rn + Hp;
+                    if (r >= den) { r -= den; ++q; }
+                    sum = hs_load<HAS_BASE>(x, ib, q);
+                    const int step = all_h ? 1 : 2;
+                    q += qn; r += rn;
+                    if (r >= den) { r -= den; ++q; }
+                    for (int h = 2; h <= Hp; h += step) {
+                        sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, q));
+                        for (int k = 0; k < step; ++k) {
+                            q += qn; r += rn;
+                            if (r >= den) { r -= den; ++q; }
+                        }
                     }
                 }
+                tile[(Hp - 1) * PITCH + lane] = (have && in_set) ? sum : NOT;
             }
-            add(Hp, have, sum);
         }
+        __syncwarp();
+        const float* row = tile + lane * PITCH;             // the 32 sums of order lane + 1
+#pragma unroll 8
+        for (int l = 0; l < 32; ++l) {
+            const float v = row[l];
+            if (v >= lo && v <= hi) {                       // false for NaN
+                const double dv = (double)v;
+                cnt += 1.0; s1 += dv; s2 += __dmul_rn(dv, dv);
+            }
+        }
+        __syncwarp();
     }
+    // the CTA's totals (shared-memory atomics), then one set of global atomics per CTA
+    __shared__ double s_acc[HS_MAX_H][3];
+    if (warp == 0) { s_acc[lane][0] = 0.0; s_acc[lane][1] = 0.0; s_acc[lane][2] = 0.0; }
+    __syncthreads();
+    if (cnt != 0.0) { atomicAdd(&s_acc[lane][0], cnt); atomicAdd(&s_acc[lane][1], s1); atomicAdd(&s_acc[lane][2], s2); }
     __syncthreads();
     if (threadIdx.x < 3 * HS_MAX_H) {
-        const int h = threadIdx.x / 3, k = threadIdx.x % 3;
-        const double v = s_acc[h][k];
-        if (v != 0.0) atomicAdd(a.acc + ((long long)s * HS_MAX_H + h) * 3 + k, v);
+        const double v = s_acc[threadIdx.x / 3][threadIdx.x % 3];
+        if (v != 0.0) atomicAdd(a.acc + (long long)s * HS_MAX_H * 3 + threadIdx.x, v);
     }
 }
 
@@ -137,4 +142,27 @@ __global__ void hs_stats_finish_kernel(const double* __restrict__ acc, int S, in
     hs_moments(a, mean, sd);
     mu[i] = a[0] > 0.0 ? __double2float_rn(mean) : 0.f;
     sigma[i] = (a[0] > 0.0 && sd > 0.0) ? __double2float_rn(sd) : 1.f;
+}
+
+// Spectrum whitening as its own pass ("further preprocessing, which includes spectrum whitening"):
+// y[s][b] = x[s][b] * inv_baseline[s][b], ONE fp32 multiply -- exactly the product the fused path forms (reading R13),
+// so hs_run_*(y, NULL) returns the bits of hs_run_*(x, inv_baseline).  16-byte streaming loads, 16-byte stores;
+// the gather of the harmonic sum then reads one array instead of two.
+__global__ void __launch_bounds__(256)
+hs_whiten_kernel(const float* __restrict__ x, const float* __restrict__ ib, float* __restrict__ y, long long in_stride,
+                 long long y_stride, int n_bins) {
+    const int s = blockIdx.y;
+    const float* xr = x + (long long)s * in_stride;
+    const float* br = ib + (long long)s * in_stride;
+    float* yr = y + (long long)s * y_stride;
+    const int n4 = n_bins >> 2;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
+        const float4 a = __ldcs(reinterpret_cast<const float4*>(xr) + i);
+        const float4 b = __ldcs(reinterpret_cast<const float4*>(br) + i);
+        reinterpret_cast<float4*>(yr)[i] = make_float4(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y), __fmul_rn(a.z, b.z), __fmul_rn(a.w, b.w));
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n_bins & 3)) {
+        const int i = (n4 << 2) + threadIdx.x;
+        yr[i] = __fmul_rn(__ldg(xr + i), __ldg(br + i));
+    }
 }

@@ -887,3 +887,33 @@ def test_2d_plans_and_1d_entry_points_do_not_mix(hs):
             hs.hs_plan_2d(1024, 3, 32)           # H <= 16
     finally:
         hs.hs_destroy(p1); hs.hs_destroy(p2)
+
+
+def test_whiten_pass_equals_fused_multiplier(hs, oracle_mod):
+    """hs_whiten then hs_run_*(y, NULL) returns the bits of hs_run_*(x, inv_baseline) (reading R13: one fp32 multiply),
+    ragged rows included; nothing beyond n_bins of a row is written."""
+    H, S, N = 32, 3, 50001
+    istr = (N + 3) & ~3
+    w = inputs.Workload("red", S, N, H, seed=4, n_pulsars=2, r_range=(100.0, 1500.0), duty_range=(0.02, 0.1), amp_range=(8.0, 12.0), red_noise=True)
+    x = torch.zeros((S, istr), device="cuda"); x[:, :N] = inputs.generate(w, "cuda")
+    ib = torch.ones((S, istr), device="cuda"); ib[:, :N] = inputs.block_median_inv_baseline(x[:, :N].contiguous())
+    y = torch.full((S, istr), float("nan"), device="cuda")
+    out = [torch.empty((S, istr), dtype=torch.float32 if k % 2 == 0 else torch.int32, device="cuda") for k in range(4)]
+    plan = hs.hs_plan(N, S, H, istr, istr, 0, 0, 0)
+    try:
+        hs.hs_whiten(plan, x, ib, y)
+        torch.cuda.synchronize()
+        assert torch.equal(y[:, :N], x[:, :N] * ib[:, :N]) and bool(torch.isnan(y[:, N:]).all())
+        mu, sg = inputs.exp1_stats("greedy", H)
+        hs.hs_run_greedy(plan, x, ib, mu, sg, out[0], out[1])
+        hs.hs_run_greedy(plan, y, None, mu, sg, out[2], out[3])
+        torch.cuda.synchronize()
+        assert torch.equal(out[0][:, :N].view(torch.int32), out[2][:, :N].view(torch.int32)) and torch.equal(out[1][:, :N], out[3][:, :N])
+        mu, sg = inputs.exp1_stats("presto", H)
+        hs.hs_run_presto(plan, x, ib, mu, sg, out[0], out[1])
+        hs.hs_run_presto(plan, y, None, mu, sg, out[2], out[3])
+        torch.cuda.synchronize()
+        # the fused path runs the coverage kernel (written order), the whitened one the tile kernel (level order)
+        assert torch.allclose(out[0][:, :N], out[2][:, :N], rtol=1e-5, atol=2e-5)
+    finally:
+        hs.hs_destroy(plan)
