@@ -14,6 +14,7 @@
 #include "hs_greedy.cuh"
 #include "hs_presto_tile.cuh"
 #include "hs_presto_farey.cuh"
+#include "hs_presto_plus.cuh"
 #include "hs_candidates.cuh"
 #include "hs_stats.cuh"
 #include "hs_2d.cuh"
@@ -217,13 +218,27 @@ hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
 }
 
 hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
-    // PRESTO_all, and PRESTO+ at H > 16 (measured: below that the coverage kernel is faster): hs_presto_farey.cuh
-    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && !io.d_mu && p->tune != HS_TUNE_GENERIC &&
-        (!(sh.flags & HS_PRESTO_ALL_ORDERS) || sh.H > 16 || p->tune == 1)) {
-        dim3 fgrid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
-        if (sh.flags & HS_PRESTO_ALL_ORDERS) hs_presto_farey_kernel<true><<<fgrid, 256, 0, stream>>>(sh, st, io);
-        else hs_presto_farey_kernel<false><<<fgrid, 256, 0, stream>>>(sh, st, io);
-        p->last_kernel = "hs_presto_farey_kernel";
+    // PRESTO_all / PRESTO+: reduced (Farey) fractions; default = the staged kernel (hs_presto_plus.cuh), tune 1 = the
+    // one-thread-per-bin Farey kernel (hs_presto_farey.cuh)
+    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && !io.d_mu && p->tune != HS_TUNE_GENERIC) {
+        const bool all_o = sh.flags & HS_PRESTO_ALL_ORDERS;
+        if (p->tune == 1 || (!all_o && p->tune != 2)) {          // measured: PRESTO_all 16.0 ms (Farey) against 19.6 ms (staged)
+            dim3 fgrid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
+            if (all_o) hs_presto_farey_kernel<true><<<fgrid, 256, 0, stream>>>(sh, st, io);
+            else hs_presto_farey_kernel<false><<<fgrid, 256, 0, stream>>>(sh, st, io);
+            p->last_kernel = "hs_presto_farey_kernel";
+        } else {
+            static std::atomic<uint64_t> opted_a{0}, opted_b{0};
+            dim3 pgrid((unsigned)((sh.n_fund + hs_plus::T - 1) / hs_plus::T), (unsigned)sh.n_spectra);
+            if (all_o) {
+                HS_CUDA(opt_in_smem(hs_presto_plus_kernel<true>, hs_plus::smem_bytes(), p->device, opted_a));
+                hs_presto_plus_kernel<true><<<pgrid, hs_plus::NT, hs_plus::smem_bytes(), stream>>>(sh, st, io);
+            } else {
+                HS_CUDA(opt_in_smem(hs_presto_plus_kernel<false>, hs_plus::smem_bytes(), p->device, opted_b));
+                hs_presto_plus_kernel<false><<<pgrid, hs_plus::NT, hs_plus::smem_bytes(), stream>>>(sh, st, io);
+            }
+            p->last_kernel = "hs_presto_plus_kernel";
+        }
         p->launches += 1;
         HS_CUDA(cudaGetLastError());
         return HS_OK;

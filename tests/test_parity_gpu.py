@@ -149,7 +149,7 @@ def test_simple_hs_exact_integer(hs, oracle_mod, flags, tune):
     assert np.all(p == 0) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
 
 
-@pytest.mark.parametrize("tune", [0, 1, 255])       # library choice / Farey kernel forced / generic kernel
+@pytest.mark.parametrize("tune", [0, 1, 2, 255])    # library choice / Farey kernel forced / staged kernel forced / generic kernel
 @pytest.mark.parametrize("flags", [ALL_HARMONICS, ALL_HARMONICS | ALL_ORDERS])
 @pytest.mark.parametrize("H", [1, 2, 5, 16, 27, 32])
 def test_presto_variants_exact_integer(hs, oracle_mod, flags, H, tune):
