@@ -917,3 +917,37 @@ def test_whiten_pass_equals_fused_multiplier(hs, oracle_mod):
         assert torch.allclose(out[0][:, :N], out[2][:, :N], rtol=1e-5, atol=2e-5)
     finally:
         hs.hs_destroy(plan)
+
+
+def test_more_than_65535_spectra(hs, oracle_mod):
+    """gridDim.y carries the spectrum index and is limited to 65 535: larger batches go out in slices (every pointer,
+    the per-spectrum statistics included, advances with the slice).  65 540 short spectra, exact integers."""
+    H, S, N = 4, 65540, 64
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(900, 4, S * N // 4, 100).reshape(S, N).contiguous().numpy()
+    s_ref, b_ref, p_ref = oracle_mod.greedy(x, H, mu, sg, 0)
+    s, b, p = run_greedy(hs, x, H, mu, sg, 0)
+    assert np.array_equal(p.view(np.uint32), p_ref) and np.array_equal(b, b_ref) and np.array_equal(s.astype(np.float64), s_ref)
+    q_ref, c_ref = oracle_mod.presto(x, H, mu, sg)
+    q, c = run_presto(hs, x, H, mu, sg)
+    assert np.array_equal(c, c_ref) and np.array_equal(q.astype(np.float64), q_ref)
+    # per-spectrum statistics from the device: spectrum s gets mu + (s % 7), so a slice that did not advance its
+    # statistics pointer would be caught; estimated statistics of the last rows against the oracle
+    dx = torch.from_numpy(x).cuda()
+    dmu = (torch.from_numpy(mu)[None, :] + (torch.arange(S) % 7)[:, None].float()).cuda().contiguous()
+    dsg = torch.from_numpy(sg)[None, :].repeat(S, 1).cuda().contiguous()
+    snr = torch.empty((S, N), dtype=torch.float32, device="cuda"); bh = torch.empty((S, N), dtype=torch.int32, device="cuda")
+    emu = torch.empty((S, H), device="cuda"); esg = torch.empty((S, H), device="cuda")
+    plan = hs.hs_plan(N, S, H)
+    try:
+        hs.hs_run_greedy_dstats(plan, dx, None, dmu, dsg, snr, bh, None)
+        work = torch.empty(hs.hs_stats_workspace_bytes(plan, 1) // 8, dtype=torch.float64, device="cuda")
+        hs.hs_estimate_stats(plan, True, dx, None, 1, 16, 3.0, 1, emu, esg, work)
+        torch.cuda.synchronize()
+    finally:
+        hs.hs_destroy(plan)
+    for srow in (0, 65534, 65535, 65536, S - 1):
+        r_s, r_b, _ = oracle_mod.greedy(x[srow], H, dmu[srow].cpu().numpy(), sg, 0)
+        assert np.array_equal(bh[srow].cpu().numpy(), r_b[0]) and np.array_equal(snr[srow].cpu().numpy().astype(np.float64), r_s[0])
+    m_r, s_r, _ = oracle_mod.estimate_stats(x[65530:], H, 0, True, 1, 16, clip=3.0, n_clip=1)
+    assert np.array_equal(emu[65530:].cpu().numpy(), m_r) and np.array_equal(esg[65530:].cpu().numpy(), s_r)
