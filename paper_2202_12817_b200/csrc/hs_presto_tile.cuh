@@ -63,6 +63,26 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     }
 }
 
+// t[p - LO] = row[p] for p = P .. HI: 16-, 8- or 4-byte loads, whichever is aligned (the row start is aligned to A words)
+// and stays inside the range
+template <int A, int LO, int P, int HI, int NW>
+__device__ __forceinline__ void load_words(const float* __restrict__ row, float (&t)[NW]) {
+    if constexpr (P <= HI) {
+        if constexpr (A >= 4 && P % 4 == 0 && P + 3 <= HI) {
+            const float4 q = *reinterpret_cast<const float4*>(row + P);
+            t[P - LO] = q.x; t[P - LO + 1] = q.y; t[P - LO + 2] = q.z; t[P - LO + 3] = q.w;
+            load_words<A, LO, P + 4, HI>(row, t);
+        } else if constexpr (A >= 2 && P % 2 == 0 && P + 1 <= HI) {
+            const float2 q = *reinterpret_cast<const float2*>(row + P);
+            t[P - LO] = q.x; t[P - LO + 1] = q.y;
+            load_words<A, LO, P + 2, HI>(row, t);
+        } else {
+            t[P - LO] = row[P];
+            load_words<A, LO, P + 1, HI>(row, t);
+        }
+    }
+}
+
 // add the term of fraction KK to the accumulators of outputs e = E0 + u, u = 0..NE-1
 // (FIRST: they are set, not added to)
 template <int KK, int E0, int NE, bool FIRST>
@@ -75,24 +95,13 @@ __device__ __forceinline__ void add_terms(const float* __restrict__ row, float (
     }
     constexpr int lo = row_off(KK, E0), hi = row_off(KK, E0 + NE - 1);
     constexpr int A = (KK % 8 == 0) ? 4 : (KK % 4 == 0) ? 2 : 1;     // words the row start is aligned to
-    constexpr int lo_al = lo & ~(A - 1);
-    constexpr int nvec = (hi - lo_al) / A + 1;
-    float t[nvec * A];
-#pragma unroll
-    for (int v = 0; v < nvec; ++v) {
-        if (A == 4) {
-            const float4 q = *reinterpret_cast<const float4*>(row + lo_al + 4 * v);
-            t[4 * v] = q.x; t[4 * v + 1] = q.y; t[4 * v + 2] = q.z; t[4 * v + 3] = q.w;
-        } else if (A == 2) {
-            const float2 q = *reinterpret_cast<const float2*>(row + lo_al + 2 * v);
-            t[2 * v] = q.x; t[2 * v + 1] = q.y;
-        } else {
-            t[v] = row[lo_al + v];
-        }
-    }
+    // exactly the words lo .. hi, by the widest aligned loads that stay inside them (the shared-memory pipe is the
+    // kernel's busiest unit: a 16-byte load that is only half used costs its full 4 wavefronts)
+    float t[hi - lo + 1];
+    load_words<A, lo, lo, hi>(row, t);
 #pragma unroll
     for (int u = 0; u < NE; ++u) {
-        const float v = t[row_off(KK, E0 + u) - lo_al];
+        const float v = t[row_off(KK, E0 + u) - lo];
         acc[u] = FIRST ? v : __fadd_rn(acc[u], v);
     }
 }
