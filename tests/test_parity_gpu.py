@@ -951,3 +951,34 @@ def test_more_than_65535_spectra(hs, oracle_mod):
         assert np.array_equal(bh[srow].cpu().numpy(), r_b[0]) and np.array_equal(snr[srow].cpu().numpy().astype(np.float64), r_s[0])
     m_r, s_r, _ = oracle_mod.estimate_stats(x[65530:], H, 0, True, 1, 16, clip=3.0, n_clip=1)
     assert np.array_equal(emu[65530:].cpu().numpy(), m_r) and np.array_equal(esg[65530:].cpu().numpy(), s_r)
+
+
+def test_host_path_many_slots_and_both_forms(hs, oracle_mod, monkeypatch):
+    """The host entry points stream the batch through two staging slots on two streams: with a 1 MiB slot
+    (HS_HOST_SLOT_MIB, unstable test knob) 20 spectra of 40 000 bins take four chunks, so slots are re-used while the
+    other stream is busy.  hs_run_both_host (one upload, both forms), with multiplier and path, against the oracle bit
+    for bit on exact integers."""
+    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
+    H, S, N = 16, 20, 40000
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(15, S, N, 63)
+    rng = np.random.default_rng(8)
+    ib = torch.from_numpy((2.0 ** rng.integers(-1, 3, size=(S, N))).astype(np.float32))
+    pin = lambda t: t.pin_memory()
+    hx, hib = pin(x), pin(ib)
+    snr_g = pin(torch.empty((S, N), dtype=torch.float32)); bh_g = pin(torch.empty((S, N), dtype=torch.int32))
+    path = pin(torch.empty((S, N), dtype=torch.int32))
+    snr_p = pin(torch.empty((S, N), dtype=torch.float32)); bh_p = pin(torch.empty((S, N), dtype=torch.int32))
+    for use_ib in (False, True):
+        plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+        try:
+            hs.hs_run_both_host(plan, hx, hib if use_ib else None, mu, sg, snr_g, bh_g, path, mu, sg, snr_p, bh_p)
+            assert hs.hs_launch_count(plan) >= 8            # four chunks x two forms
+        finally:
+            hs.hs_destroy(plan)
+        kw = dict(inv_baseline=ib.numpy()) if use_ib else {}
+        s_ref, b_ref, p_ref = oracle_mod.greedy(x.numpy(), H, mu, sg, 0, **kw)
+        assert np.array_equal(path.numpy().view(np.uint32), p_ref) and np.array_equal(bh_g.numpy(), b_ref)
+        assert np.array_equal(snr_g.numpy().astype(np.float64), s_ref)
+        q_ref, c_ref = oracle_mod.presto(x.numpy(), H, mu, sg, 0, **kw)
+        assert np.array_equal(bh_p.numpy(), c_ref) and np.array_equal(snr_p.numpy().astype(np.float64), q_ref)
