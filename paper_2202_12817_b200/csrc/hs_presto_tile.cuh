@@ -15,10 +15,11 @@
 // known when the kernel is compiled: 147 elements for its 16 outputs instead of 17 x 16 separate loads.
 //
 // Data movement of a CTA tile of T = 512 W outputs (W pairs of warps):
-//   * 15 spans (all fractions but kk = 32 and 16) are copied into shared memory as they are by one 1-D bulk
+//   * 14 spans (all fractions but kk = 32, 16 and 8) are copied into shared memory as they are by one 1-D bulk
 //     async copy each (TMA engine, cp.async.bulk -> UBLKCP), completing on one mbarrier; a lane stride of
 //     kk/2 words makes the vector loads LDS.128 / .64 / .32 bank-conflict free for every one of them;
-//   * kk = 32 (x[n] itself) and kk = 16 would bank-conflict at lane strides of 16 / 8 words, and a lane's words
+//   * kk = 32 (x[n] itself) and kk = 16 would bank-conflict at lane strides of 16 / 8 words (kk = 8 joins them so that
+//     the tile's shared memory drops under 27.5 KB and an SM holds 8 CTAs instead of 7), and a lane's words
 //     are contiguous in global memory too: they are loaded straight into registers (LDG.256 / LDG.128) while
 //     the bulk copies are in flight, which also keeps 12 B/bin off the shared-memory pipe;
 //   * two warps share each 512-output warp tile (one takes outputs e < 8 of every lane's 16, the other e >= 8):
@@ -42,13 +43,14 @@ __host__ __device__ constexpr int frac_kk(int f) {
 }
 // words of shared memory of the span of fraction kk of a CTA tile of W warp tiles (+ 4: the word shared with the next tile)
 __host__ __device__ constexpr int span_words(int kk, int W) { return 16 * kk * W + 4; }
-// stage layout: fractions 2 .. NF-1 (kk = 8, 4, 24, 2, ...) back to back; 0 (kk = 32) and 1 (kk = 16) stay in registers
+// stage layout: fractions 3 .. NF-1 (kk = 4, 24, 2, ...) back to back; 0 (kk = 32), 1 (kk = 16) and 2 (kk = 8) stay in registers
+constexpr int F_SMEM = 3;                   // first fraction that goes through shared memory
 __host__ __device__ constexpr int span_off(int f, int W) {
     int o = 0;
-    for (int g = 2; g < f; ++g) o += span_words(frac_kk(g), W);
+    for (int g = F_SMEM; g < f; ++g) o += span_words(frac_kk(g), W);
     return o;
 }
-__host__ __device__ constexpr int smem_words(int L, int W) { return n_frac(L) > 2 ? span_off(n_frac(L), W) : 4; }
+__host__ __device__ constexpr int smem_words(int L, int W) { return n_frac(L) > F_SMEM ? span_off(n_frac(L), W) : 4; }
 
 // offset of output e in the row of fraction kk (kk even)
 __host__ __device__ constexpr int row_off(int kk, int e) { return (kk * e + 16) >> 5; }
@@ -127,14 +129,16 @@ __device__ __forceinline__ const float* row_ptr(const float* __restrict__ sm, in
 
 // the words of 8 outputs of a lane that come straight from global memory:
 // xr = x[n .. n + 8) (fraction 32/32), yr = x[i16 .. i16 + 5) (fraction 16/32: output u reads yr[(u + 1) >> 1])
+// zr = x[i8 .. i8 + 3) (fraction 8/32: output u reads zr[(u + 2) >> 2])
 struct Direct {
     float xr[8];
     float yr[5];
+    float zr[3];
 };
 
 template <int L>
-__device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__ x, const float* __restrict__ x16, int N, int n, int i16,
-                                            bool interior, bool al32) {     // x16: the row fraction 16/32 reads from (x itself in 1-D)
+__device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__ x, const float* __restrict__ x16, const float* __restrict__ x8,
+                                            int N, int n, int i16, int i8, bool interior, bool al32) {   // x16, x8: the rows fractions 16/32, 8/32 read from (x itself in 1-D)
     if (interior) {
         if (al32) {
             asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
@@ -151,12 +155,20 @@ __device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__
                          : "=f"(d.yr[0]), "=f"(d.yr[1]), "=f"(d.yr[2]), "=f"(d.yr[3]) : "l"(x16 + i16));
             asm volatile("ld.global.nc.f32 %0, [%1];\n" : "=f"(d.yr[4]) : "l"(x16 + i16 + 4));
         }
+        if (L >= 2) {
+            asm volatile("ld.global.nc.v2.f32 {%0,%1}, [%2];\n" : "=f"(d.zr[0]), "=f"(d.zr[1]) : "l"(x8 + i8));
+            asm volatile("ld.global.nc.f32 %0, [%1];\n" : "=f"(d.zr[2]) : "l"(x8 + i8 + 2));
+        }
     } else {                                                 // the last tile of a row: element-wise, zero beyond the end
 #pragma unroll
         for (int u = 0; u < 8; ++u) d.xr[u] = (n + u < N) ? __ldg(x + n + u) : 0.f;
         if (L >= 1) {
 #pragma unroll
             for (int u = 0; u < 5; ++u) d.yr[u] = (i16 + u < N) ? __ldg(x16 + i16 + u) : 0.f;
+        }
+        if (L >= 2) {
+#pragma unroll
+            for (int u = 0; u < 3; ++u) d.zr[u] = (i8 + u < N) ? __ldg(x8 + i8 + u) : 0.f;
         }
     }
 }
@@ -175,7 +187,8 @@ __device__ __forceinline__ void chain8(const float* __restrict__ sm, const HsSta
         close_level<2, 8>(st, S, add, best, bh);
     }
     if (L >= 2) {
-        add_terms<8, E0, 8, true>(row_ptr<2, W>(sm, w, lane), add);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) add[u] = d.zr[(u + 2) >> 2];
         close_level<4, 8>(st, S, add, best, bh);
     }
     if (L >= 3) {
@@ -233,7 +246,8 @@ template <int L, int W, bool DSTATS = false, bool TWOD = false>
 __global__ void __launch_bounds__(64 * W)
 hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     using namespace hs_tile;
-    __shared__ HsStats s_st;
+    __shared__ float s_st_raw[DSTATS ? sizeof(HsStats) / 4 : 1];     // only the per-spectrum-statistics build pays for it
+    HsStats& s_st = *reinterpret_cast<HsStats*>(s_st_raw);
     if (DSTATS) hs_load_dstats(s_st, io, blockIdx.y, sh.H);
     const HsStats& st = DSTATS ? s_st : st_param;
     constexpr int NF = n_frac(L);
@@ -250,7 +264,7 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
         return TWOD ? io.x + (long long)(((kk * zq + 16) >> 5) + sh.Z) * sh.in_stride : x;
     };
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (NF > 2) {
+    if (NF > F_SMEM) {
         if (threadIdx.x == 0) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(smem_u32(&bar)) : "memory");
             asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -262,13 +276,13 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             const long long lim = sh.in_stride;
             unsigned total = 0;
 #pragma unroll
-            for (int f = 2; f < NF; ++f) {
+            for (int f = F_SMEM; f < NF; ++f) {
                 const long long room = lim - (long long)frac_kk(f) * b0;
                 total += 4u * (unsigned)max(0ll, min((long long)span_words(frac_kk(f), W), room));
             }
             asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_u32(&bar)), "r"(total) : "memory");
 #pragma unroll
-            for (int f = 2; f < NF; ++f) {
+            for (int f = F_SMEM; f < NF; ++f) {
                 const int kk = frac_kk(f);
                 const long long room = lim - (long long)kk * b0;
                 const unsigned bytes = 4u * (unsigned)max(0ll, min((long long)span_words(kk, W), room));
@@ -282,9 +296,9 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int w = warp >> 1, half = warp & 1;
     const int nw = n0 + TILE * w;
     Direct d;
-    load_direct<L>(d, x, frac_row(16), N, nw + 16 * lane + 8 * half, nw / 2 + 8 * lane + 4 * half, nw + TILE + 8 <= N,
-                   (reinterpret_cast<uintptr_t>(x) & 31u) == 0);
-    if (NF > 2) mbar_wait(smem_u32(&bar), 0);
+    load_direct<L>(d, x, frac_row(16), frac_row(8), N, nw + 16 * lane + 8 * half, nw / 2 + 8 * lane + 4 * half,
+                   nw / 4 + 4 * lane + 2 * half, nw + TILE + 8 <= N, (reinterpret_cast<uintptr_t>(x) & 31u) == 0);
+    if (NF > F_SMEM) mbar_wait(smem_u32(&bar), 0);
     float best[8];
     int bh[8];
     if (half == 0) chain8<L, 0, W>(sm, st, w, lane, d, best, bh);
