@@ -227,6 +227,16 @@ typedef struct {
 hs_status hs_find_candidates(hs_plan_t plan, const float* d_snr, const int32_t* d_best_h, float threshold,
                              hs_candidate* d_out, int64_t capacity, uint64_t* d_count, void* cuda_stream);
 
+/* The search as one call on HOST buffers: the spectra are uploaded once (in groups of rows through the plan's staging
+ * slots, two streams), both forms run on the device, their outputs are thresholded and compacted THERE, and only the two
+ * candidate lists travel back -- the per-bin outputs never leave the device.  Lists as hs_find_candidates defines them
+ * (unspecified order; *h_count_* = the number of qualifying bins, which may exceed the capacity: then only `capacity`
+ * records were stored).  h_cand_* are HOST arrays.  Synchronous.  The plan owns the device lists it compacts into. */
+hs_status hs_search_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline,
+                         const float* mu_greedy, const float* sigma_greedy, const float* mu_presto, const float* sigma_presto,
+                         float threshold, hs_candidate* h_cand_greedy, int64_t capacity_greedy, uint64_t* h_count_greedy,
+                         hs_candidate* h_cand_presto, int64_t capacity_presto, uint64_t* h_count_presto);
+
 /* UNSTABLE, diagnostics only (not part of the method's interface; values may change between versions):
  * selects a kernel variant for the plan's later runs.  0 = the library's choice; 255 = the plain
  * one-thread-per-bin coverage kernels.  Every variant computes the results defined above. */

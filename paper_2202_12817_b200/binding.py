@@ -26,7 +26,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
-           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes", "hs_whiten",
+           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes", "hs_whiten", "hs_search_host",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -81,6 +81,8 @@ def load() -> ctypes.CDLL:
     lib.hs_run_presto_dstats.restype = ctypes.c_int
     lib.hs_estimate_stats.argtypes = [vp, i32, vp, vp, i64, i64, ctypes.c_float, i32, vp, vp, vp, i64, vp]
     lib.hs_estimate_stats.restype = ctypes.c_int
+    lib.hs_search_host.argtypes = [vp, vp, vp, fp, fp, fp, fp, ctypes.c_float, vp, i64, vp, vp, i64, vp]
+    lib.hs_search_host.restype = ctypes.c_int
     lib.hs_whiten.argtypes = [vp, vp, vp, vp, vp]
     lib.hs_whiten.restype = ctypes.c_int
     lib.hs_stats_workspace_bytes.argtypes = [vp, i32]
@@ -218,6 +220,19 @@ def hs_whiten(plan, d_spectra: torch.Tensor, d_inv_baseline: torch.Tensor, d_whi
         stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
     _check(lib.hs_whiten(plan, _dptr(d_spectra, torch.float32, "d_spectra"), _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"),
                          _dptr(d_whitened, torch.float32, "d_whitened"), stream), "hs_whiten")
+
+
+def hs_search_host(plan, h_spectra, h_inv_baseline, mu_greedy, sigma_greedy, mu_presto, sigma_presto, threshold: float,
+                   h_cand_greedy: torch.Tensor, h_cand_presto: torch.Tensor):
+    """h_cand_*: CPU int32 tensors [capacity, 4] (spectrum, bin, snr bits, best_h).  Returns (count_greedy, count_presto)."""
+    lib = load()
+    cg, cp = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(lib.hs_search_host(plan, _hptr(h_spectra, torch.float32, "h_spectra"), _hptr(h_inv_baseline, torch.float32, "h_inv_baseline"),
+                              _farr(mu_greedy), _farr(sigma_greedy), _farr(mu_presto), _farr(sigma_presto), threshold,
+                              _hptr(h_cand_greedy, torch.int32, "h_cand_greedy"), h_cand_greedy.shape[0], ctypes.byref(cg),
+                              _hptr(h_cand_presto, torch.int32, "h_cand_presto"), h_cand_presto.shape[0], ctypes.byref(cp)),
+           "hs_search_host")
+    return int(cg.value), int(cp.value)
 
 
 def hs_stats_workspace_bytes(plan, n_clip: int) -> int:

@@ -37,6 +37,9 @@ struct HostStage {          // staging for the *_host entry points (created on f
     float* d_snr[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};     // [slot][form]: form 0 = first output set, 1 = second (hs_run_both_host)
     int32_t* d_bh[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
     uint32_t* d_path[2] = {nullptr, nullptr};
+    HsCandidate* d_cand = nullptr;           // hs_search_host: greedy list followed by the PRESTO list
+    int64_t cand_cap = 0;
+    uint64_t* d_cand_count = nullptr;        // [2]
 };
 
 }  // namespace
@@ -308,6 +311,9 @@ void free_stage(HostStage& g) {
         if (g.stream[i]) cudaStreamDestroy(g.stream[i]);
         g.d_in[i] = g.d_base[i] = nullptr; g.d_path[i] = nullptr; g.stream[i] = nullptr;
     }
+    if (g.d_cand) cudaFree(g.d_cand);
+    if (g.d_cand_count) cudaFree(g.d_cand_count);
+    g.d_cand = nullptr; g.d_cand_count = nullptr; g.cand_cap = 0;
     g.ready = false;
 }
 
@@ -422,6 +428,26 @@ hs_status launch_presto_tile_2d(hs_plan_s* p, const HsStats& st, const HsIO& io,
     p->last_kernel = "hs_presto_tile_kernel<W=2,2d>";
     p->launches += 1;
     HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+// threshold + compaction of `rows` output rows whose first spectrum has index s_base; appends to d_out / d_count
+hs_status launch_candidates(hs_plan_s* plan, const float* d_snr, const int32_t* d_best_h, long long n_rows, long long s_base,
+                            float threshold, hs_candidate* d_out, int64_t capacity, uint64_t* d_count, cudaStream_t stream) {
+    const HsShape& sh = plan->shape;
+    if (sh.n_fund == 0) return HS_OK;
+    const long long n4 = (sh.n_fund + 3) / 4;
+    for (long long s0 = 0; s0 < n_rows; s0 += HS_MAX_GRID_Y) {
+        const int rows = (int)std::min<long long>(HS_MAX_GRID_Y, n_rows - s0);
+        // a few waves of 256-thread CTAs per spectrum row, grid-stride inside the row
+        const long long per_row = std::max(1ll, std::min((n4 + 255) / 256, (long long)std::max(1, plan->sm_count * 64 / rows + 1)));
+        dim3 grid((unsigned)per_row, (unsigned)rows);
+        hs_candidates_kernel<256><<<grid, 256, 0, stream>>>(d_snr + s0 * sh.out_stride, d_best_h + s0 * sh.out_stride, sh.out_stride,
+                                                            (int)sh.n_fund, (int)(s_base + s0), threshold, reinterpret_cast<HsCandidate*>(d_out),
+                                                            (unsigned long long)capacity, reinterpret_cast<unsigned long long*>(d_count));
+        plan->launches += 1;
+        HS_CUDA(cudaGetLastError());
+    }
     return HS_OK;
 }
 
@@ -706,24 +732,76 @@ hs_status hs_find_candidates(hs_plan_t plan, const float* d_snr, const int32_t* 
     if (!aligned16(d_snr) || !aligned16(d_best_h) || (d_out && !aligned16(d_out)) || (reinterpret_cast<uintptr_t>(d_count) & 7u))
         return HS_ERR_INVALID_ARG;
     if (!(threshold == threshold)) return HS_ERR_INVALID_ARG;
-    const HsShape& sh = plan->shape;
     DeviceGuard guard(plan->device);
     HS_CUDA(guard.err);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     HS_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint64_t), stream));
-    if (sh.n_fund == 0) return HS_OK;
-    const long long n4 = (sh.n_fund + 3) / 4;
-    for (long long s0 = 0; s0 < sh.n_spectra; s0 += HS_MAX_GRID_Y) {
-        const int rows = (int)std::min<long long>(HS_MAX_GRID_Y, sh.n_spectra - s0);
-        // a few waves of 256-thread CTAs per spectrum row, grid-stride inside the row
-        const long long per_row = std::max(1ll, std::min((n4 + 255) / 256, (long long)std::max(1, plan->sm_count * 64 / rows + 1)));
-        dim3 grid((unsigned)per_row, (unsigned)rows);
-        hs_candidates_kernel<256><<<grid, 256, 0, stream>>>(d_snr + s0 * sh.out_stride, d_best_h + s0 * sh.out_stride, sh.out_stride,
-                                                            (int)sh.n_fund, (int)s0, threshold, reinterpret_cast<HsCandidate*>(d_out),
-                                                            (unsigned long long)capacity, reinterpret_cast<unsigned long long*>(d_count));
-        plan->launches += 1;
-        HS_CUDA(cudaGetLastError());
+    return launch_candidates(plan, d_snr, d_best_h, plan->shape.n_spectra, 0, threshold, d_out, capacity, d_count, stream);
+}
+
+hs_status hs_search_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline,
+                         const float* mu_greedy, const float* sigma_greedy, const float* mu_presto, const float* sigma_presto,
+                         float threshold, hs_candidate* h_cand_greedy, int64_t capacity_greedy, uint64_t* h_count_greedy,
+                         hs_candidate* h_cand_presto, int64_t capacity_presto, uint64_t* h_count_presto) {
+    if (!plan || plan->two_d || !h_spectra || !h_count_greedy || !h_count_presto || capacity_greedy < 0 || capacity_presto < 0 ||
+        (capacity_greedy > 0 && !h_cand_greedy) || (capacity_presto > 0 && !h_cand_presto) || !(threshold == threshold))
+        return HS_ERR_INVALID_ARG;
+    HsStats st_g, st_p;
+    hs_status rc = fill_stats(plan, mu_greedy, sigma_greedy, &st_g);
+    if (rc != HS_OK) return rc;
+    if ((rc = fill_stats(plan, mu_presto, sigma_presto, &st_p)) != HS_OK) return rc;
+    DeviceGuard guard(plan->device);
+    HS_CUDA(guard.err);
+    if ((rc = ensure_stage(plan, h_inv_baseline != nullptr, false, false)) != HS_OK) return rc;
+    HostStage& g = plan->stage;
+    const HsShape& full = plan->shape;
+    // candidate buffers and counters on the device (owned by the plan's host path; grown on demand)
+    const int64_t need = capacity_greedy + capacity_presto;
+    if (g.cand_cap < need || !g.d_cand_count) {
+        if (g.d_cand) cudaFree(g.d_cand);
+        g.d_cand = nullptr; g.cand_cap = 0;
+        if (!g.d_cand_count && cudaMalloc(&g.d_cand_count, 2 * sizeof(uint64_t)) != cudaSuccess) { (void)cudaGetLastError(); return HS_ERR_ALLOC; }
+        if (need > 0 && cudaMalloc(&g.d_cand, (size_t)need * sizeof(HsCandidate)) != cudaSuccess) { (void)cudaGetLastError(); return HS_ERR_ALLOC; }
+        g.cand_cap = need;
     }
+    HS_CUDA(cudaMemsetAsync(g.d_cand_count, 0, 2 * sizeof(uint64_t), g.stream[0]));
+    HS_CUDA(cudaStreamSynchronize(g.stream[0]));                    // both streams append to the same counters
+    hs_candidate* d_cg = reinterpret_cast<hs_candidate*>(g.d_cand);
+    hs_candidate* d_cp = d_cg ? d_cg + capacity_greedy : nullptr;
+    hs_status result = HS_OK;
+    int chunk = 0;
+    for (int s0 = 0; s0 < full.n_spectra && result == HS_OK; s0 += g.rows, ++chunk) {
+        const int i = chunk & 1;
+        const int rows = std::min(g.rows, full.n_spectra - s0);
+        cudaStream_t stm = g.stream[i];
+        HsShape sh = full;
+        sh.n_spectra = rows;
+        cudaError_t e = cudaMemcpy2DAsync(g.d_in[i], full.in_stride * 4, h_spectra + (long long)s0 * full.in_stride, full.in_stride * 4,
+                                          full.n_bins * 4, rows, cudaMemcpyHostToDevice, stm);
+        if (e == cudaSuccess && h_inv_baseline)
+            e = cudaMemcpy2DAsync(g.d_base[i], full.in_stride * 4, h_inv_baseline + (long long)s0 * full.in_stride, full.in_stride * 4,
+                                  full.n_bins * 4, rows, cudaMemcpyHostToDevice, stm);
+        if (e != cudaSuccess) { result = cuda_fail(e); break; }
+        HsIO io{g.d_in[i], h_inv_baseline ? g.d_base[i] : nullptr, g.d_snr[i][0], g.d_bh[i][0], nullptr, nullptr, nullptr};
+        if ((result = launch_greedy(plan, sh, st_g, io, stm)) != HS_OK) break;
+        if ((result = launch_candidates(plan, g.d_snr[i][0], g.d_bh[i][0], rows, s0, threshold, d_cg, capacity_greedy,
+                                        g.d_cand_count, stm)) != HS_OK) break;
+        if ((result = launch_presto(plan, sh, st_p, io, stm)) != HS_OK) break;
+        if ((result = launch_candidates(plan, g.d_snr[i][0], g.d_bh[i][0], rows, s0, threshold, d_cp, capacity_presto,
+                                        g.d_cand_count + 1, stm)) != HS_OK) break;
+    }
+    for (int i = 0; i < 2; ++i) {
+        cudaError_t e = cudaStreamSynchronize(g.stream[i]);
+        if (e != cudaSuccess && result == HS_OK) result = cuda_fail(e);
+    }
+    if (result != HS_OK) return result;
+    uint64_t counts[2] = {0, 0};
+    HS_CUDA(cudaMemcpy(counts, g.d_cand_count, sizeof(counts), cudaMemcpyDeviceToHost));
+    *h_count_greedy = counts[0];
+    *h_count_presto = counts[1];
+    const uint64_t ng = std::min<uint64_t>(counts[0], (uint64_t)capacity_greedy), np_ = std::min<uint64_t>(counts[1], (uint64_t)capacity_presto);
+    if (ng) HS_CUDA(cudaMemcpy(h_cand_greedy, d_cg, ng * sizeof(hs_candidate), cudaMemcpyDeviceToHost));
+    if (np_) HS_CUDA(cudaMemcpy(h_cand_presto, d_cp, np_ * sizeof(hs_candidate), cudaMemcpyDeviceToHost));
     return HS_OK;
 }
 

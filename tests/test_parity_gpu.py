@@ -982,3 +982,33 @@ def test_host_path_many_slots_and_both_forms(hs, oracle_mod, monkeypatch):
         assert np.array_equal(snr_g.numpy().astype(np.float64), s_ref)
         q_ref, c_ref = oracle_mod.presto(x.numpy(), H, mu, sg, 0, **kw)
         assert np.array_equal(bh_p.numpy(), c_ref) and np.array_equal(snr_p.numpy().astype(np.float64), q_ref)
+
+
+def test_search_host_candidates_only(hs, oracle_mod, monkeypatch):
+    """hs_search_host: one upload, both forms, threshold + compaction on the device, only the lists come back.  Against the
+    plain definition applied to the oracle's outputs (exact integers, so every snr is exact), several staging chunks,
+    and a capacity smaller than the list."""
+    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
+    H, S, N = 16, 20, 40000
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(16, S, N, 63)
+    s_ref, b_ref, _ = oracle_mod.greedy(x.numpy(), H, mu, sg, 0)
+    q_ref, c_ref = oracle_mod.presto(x.numpy(), H, mu, sg, 0)
+    T = float(np.float32(min(np.sort(s_ref.ravel())[-5000], np.sort(q_ref.ravel())[-5000])))     # at least 5 000 hits per form
+    hx = x.pin_memory()
+    cg = torch.full((1 << 20, 4), -1, dtype=torch.int32); cp = torch.full((1 << 20, 4), -1, dtype=torch.int32)
+    plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+    try:
+        ng, np_ = hs.hs_search_host(plan, hx, None, mu, sg, mu, sg, T, cg, cp)
+        small = torch.full((5, 4), -1, dtype=torch.int32)
+        ng2, _ = hs.hs_search_host(plan, hx, None, mu, sg, mu, sg, T, small, cp)
+    finally:
+        hs.hs_destroy(plan)
+    for got, n, (sr, br) in ((cg, ng, (s_ref, b_ref)), (cp, np_, (q_ref, c_ref))):
+        ref, ref_snr = oracle_mod.candidates(sr.astype(np.float32), br, T)
+        assert n == ref.shape[0] and 10 < n < got.shape[0]
+        g = got[:n].numpy()
+        g = g[np.lexsort((g[:, 1], g[:, 0]))]
+        assert np.array_equal(g[:, [0, 1, 3]].astype(np.int64), ref)
+        assert np.array_equal(g[:, 2].copy().view(np.float32).astype(np.float64), ref_snr)
+    assert ng2 == ng and bool((small[:, 0] >= 0).all())
