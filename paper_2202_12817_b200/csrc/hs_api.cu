@@ -223,7 +223,9 @@ hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st,
 hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     // PRESTO_all / PRESTO+: reduced (Farey) fractions; default = the staged kernel (hs_presto_plus.cuh), tune 1 = the
     // one-thread-per-bin Farey kernel (hs_presto_farey.cuh)
-    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && !io.d_mu && p->tune != HS_TUNE_GENERIC) {
+    // (PRESTO+ at H <= 4 is 10 terms per bin: the coverage kernel is faster there, 70 against 56 Gbin/s on 1024 x 2^17)
+    if ((sh.flags & HS_PRESTO_ALL_HARMONICS) && !io.inv_base && !io.d_mu && p->tune != HS_TUNE_GENERIC &&
+        !((sh.flags & HS_PRESTO_ALL_ORDERS) && sh.H <= 4 && p->tune == 0)) {
         const bool all_o = sh.flags & HS_PRESTO_ALL_ORDERS;
         if (p->tune == 1 || (!all_o && p->tune != 2)) {          // measured: PRESTO_all 16.0 ms (Farey) against 19.6 ms (staged)
             dim3 fgrid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);
