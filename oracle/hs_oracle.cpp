@@ -60,7 +60,9 @@
 // (PAPER.md:170, 172), P5 brute force on tiny spectra (exact rational rounding; path-tree
 // enumeration), P6 invariants, P7 exact-integer spectra, P8 Exp(1) noise statistics.
 // Parity unpinned by anything the paper prints: R3 (tie rule of Round), R4 (band edge),
-// R6 (tie-breaks); they are fixed by the readings above.
+// R6 (tie-breaks), R14 (what GetMeanStdev() estimates) and R15 (the 2-D sums: the paper defines none);
+// they are fixed by the readings above and pinned against independent restatements only
+// (numpy moments of numpy gathers; exact-rational brute force; the z = 0 row = the 1-D sums).
 // =====================================================================================
 #include <algorithm>
 #include <cmath>
