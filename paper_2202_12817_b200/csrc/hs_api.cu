@@ -188,19 +188,20 @@ hs_status launch_greedy_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
     return HS_OK;
 }
 
-template <int L, int W>
+template <int L, int W, bool SPLIT = false>
 hs_status launch_presto_tile_L(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     constexpr int smem = 4 * hs_tile::smem_words(L, W);
     static std::atomic<uint64_t> opted{0};              // per instantiation, one bit per device
     static std::atomic<uint64_t> opted_ds{0};
     constexpr int T = hs_tile::TILE * W;
+    constexpr int NTHR = 64 * W;
     dim3 grid((unsigned)((sh.n_fund + T - 1) / T), (unsigned)sh.n_spectra);
     if (io.d_mu) {
-        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, true>, smem, p->device, opted_ds));
-        hs_presto_tile_kernel<L, W, true><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, true, false, SPLIT>, smem, p->device, opted_ds));
+        hs_presto_tile_kernel<L, W, true, false, SPLIT><<<grid, NTHR, smem, stream>>>(sh, st, io);
     } else {
-        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, false>, smem, p->device, opted));
-        hs_presto_tile_kernel<L, W, false><<<grid, 64 * W, smem, stream>>>(sh, st, io);
+        HS_CUDA(opt_in_smem(hs_presto_tile_kernel<L, W, false, false, SPLIT>, smem, p->device, opted));
+        hs_presto_tile_kernel<L, W, false, false, SPLIT><<<grid, NTHR, smem, stream>>>(sh, st, io);
     }
     p->last_kernel = W == 2 ? "hs_presto_tile_kernel<W=2>" : W == 1 ? "hs_presto_tile_kernel<W=1>" : "hs_presto_tile_kernel<W=3>";
     p->launches += 1;
@@ -208,15 +209,15 @@ hs_status launch_presto_tile_L(hs_plan_s* p, const HsShape& sh, const HsStats& s
     return HS_OK;
 }
 
-template <int W>
+template <int W, bool SPLIT = false>
 hs_status launch_presto_tile(hs_plan_s* p, const HsShape& sh, const HsStats& st, const HsIO& io, cudaStream_t stream) {
     switch (floor_log2(sh.H)) {
-        case 0: return launch_presto_tile_L<0, W>(p, sh, st, io, stream);
-        case 1: return launch_presto_tile_L<1, W>(p, sh, st, io, stream);
-        case 2: return launch_presto_tile_L<2, W>(p, sh, st, io, stream);
-        case 3: return launch_presto_tile_L<3, W>(p, sh, st, io, stream);
-        case 4: return launch_presto_tile_L<4, W>(p, sh, st, io, stream);
-        default: return launch_presto_tile_L<5, W>(p, sh, st, io, stream);
+        case 0: return launch_presto_tile_L<0, W, SPLIT>(p, sh, st, io, stream);
+        case 1: return launch_presto_tile_L<1, W, SPLIT>(p, sh, st, io, stream);
+        case 2: return launch_presto_tile_L<2, W, SPLIT>(p, sh, st, io, stream);
+        case 3: return launch_presto_tile_L<3, W, SPLIT>(p, sh, st, io, stream);
+        case 4: return launch_presto_tile_L<4, W, SPLIT>(p, sh, st, io, stream);
+        default: return launch_presto_tile_L<5, W, SPLIT>(p, sh, st, io, stream);
     }
 }
 
@@ -254,7 +255,8 @@ hs_status launch_presto_slice(hs_plan_s* p, const HsShape& sh, const HsStats& st
         switch (io.d_mu ? 0u : p->tune) {                    // measured on cfg3: W = 2 3.06 ms, W = 3 3.03 ms, W = 1 3.69 ms
             case 50: return launch_presto_tile<1>(p, sh, st, io, stream);
             case 52: return launch_presto_tile<3>(p, sh, st, io, stream);
-            default: return launch_presto_tile<2>(p, sh, st, io, stream);
+            case 53: return launch_presto_tile<2, false>(p, sh, st, io, stream);            // one mbarrier for all spans
+            default: return sh.H >= 32 ? launch_presto_tile<2, true>(p, sh, st, io, stream) : launch_presto_tile<2, false>(p, sh, st, io, stream);
         }
     }
     dim3 grid((unsigned)((sh.n_fund + 255) / 256), (unsigned)sh.n_spectra);

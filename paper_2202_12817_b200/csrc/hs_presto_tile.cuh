@@ -175,9 +175,10 @@ __device__ __forceinline__ void load_direct(Direct& d, const float* __restrict__
 
 // all levels for outputs e = E0 + u, u < 8, of the lane, level by level:
 // S_{2H'} = S_{H'} + (the new terms of the level, summed first)
-template <int L, int E0, int W>
+struct NoWait { __device__ __forceinline__ void operator()() const {} };
+template <int L, int E0, int W, class BeforeL5 = NoWait>
 __device__ __forceinline__ void chain8(const float* __restrict__ sm, const HsStats& st, int w, int lane, const Direct& d,
-                                       float (&best)[8], int (&bh)[8]) {
+                                       float (&best)[8], int (&bh)[8], BeforeL5 before_l5 = NoWait()) {
     float S[8], add[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) { S[u] = d.xr[u]; best[u] = hs_snr(S[u], st.nmis[0], st.inv_sigma[0]); bh[u] = 1; }   // H' = 1: x[n]
@@ -204,6 +205,7 @@ __device__ __forceinline__ void chain8(const float* __restrict__ sm, const HsSta
         close_level<16, 8>(st, S, add, best, bh);
     }
     if (L >= 5) {
+        before_l5();                                        // the level-5 spans may complete on a barrier of their own
         add_terms<1, E0, 8, true>(row_ptr<9, W>(sm, w, lane), add);
         add_terms<6, E0, 8, false>(row_ptr<10, W>(sm, w, lane), add);
         add_terms<10, E0, 8, false>(row_ptr<11, W>(sm, w, lane), add);
@@ -242,7 +244,10 @@ __device__ __forceinline__ void store8(float* __restrict__ ps, int* __restrict__
 // TWOD (hs_plan_2d, reading R15): blockIdx.y is the row z + Z of an f-fdot plane and the term of fraction kk/32 is read
 // from row Round(kk z / 32) = (kk z + 16) >> 5 (arithmetic shift = floor: half up also for negative z) -- the same
 // for the whole tile, so every span is still one contiguous copy, only from its own row.
-template <int L, int W, bool DSTATS = false, bool TWOD = false>
+// SPLIT: the spans of levels 2-4 (issued first) and of level 5 complete on separate mbarriers, so the first 9 terms are
+// added while the 8 longest spans are still landing (2.97 against 3.01 ms at H = 32; no gain below).  A warp of its own
+// for the issue, and two issuing threads with a barrier each, were measured too: 2.96-3.05 ms, not kept.
+template <int L, int W, bool DSTATS = false, bool TWOD = false, bool SPLIT = false>
 __global__ void __launch_bounds__(64 * W)
 hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant__ HsStats st_param, HsIO io) {
     using namespace hs_tile;
@@ -253,7 +258,8 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     constexpr int NF = n_frac(L);
     extern __shared__ float4 hs_tile_smem4[];
     float* sm = reinterpret_cast<float*>(hs_tile_smem4);
-    __shared__ unsigned long long bar;
+    __shared__ unsigned long long bar[2];
+    constexpr int F5 = 9;                                   // first fraction of level 5
     const int s = blockIdx.y;
     const int N = (int)sh.n_bins, n_fund = (int)sh.n_fund;
     const int n0 = blockIdx.x * (TILE * W);
@@ -266,7 +272,8 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (NF > F_SMEM) {
         if (threadIdx.x == 0) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(smem_u32(&bar)) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(smem_u32(&bar[0])) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(smem_u32(&bar[1])) : "memory");
             asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         }
         __syncthreads();                                    // barrier initialised; the other warps go on to their own loads
@@ -274,13 +281,15 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
             // A span is cut at the end of the row's allocation (in_stride is a multiple of 4 words, so the byte count
             // stays a multiple of 16): words beyond n_bins only ever feed outputs that do not exist.
             const long long lim = sh.in_stride;
-            unsigned total = 0;
+            unsigned total[2] = {0, 0};
 #pragma unroll
             for (int f = F_SMEM; f < NF; ++f) {
                 const long long room = lim - (long long)frac_kk(f) * b0;
-                total += 4u * (unsigned)max(0ll, min((long long)span_words(frac_kk(f), W), room));
+                total[(SPLIT && f >= F5) ? 1 : 0] += 4u * (unsigned)max(0ll, min((long long)span_words(frac_kk(f), W), room));
             }
-            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_u32(&bar)), "r"(total) : "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_u32(&bar[0])), "r"(total[0]) : "memory");
+            if (SPLIT && NF > F5)
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(smem_u32(&bar[1])), "r"(total[1]) : "memory");
 #pragma unroll
             for (int f = F_SMEM; f < NF; ++f) {
                 const int kk = frac_kk(f);
@@ -288,7 +297,8 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
                 const unsigned bytes = 4u * (unsigned)max(0ll, min((long long)span_words(kk, W), room));
                 if (bytes)
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                                 :: "r"(smem_u32(sm + span_off(f, W))), "l"(frac_row(kk) + kk * b0), "r"(bytes), "r"(smem_u32(&bar)) : "memory");
+                                 :: "r"(smem_u32(sm + span_off(f, W))), "l"(frac_row(kk) + kk * b0), "r"(bytes),
+                                    "r"(smem_u32(&bar[(SPLIT && f >= F5) ? 1 : 0])) : "memory");
             }
         }
     }
@@ -298,11 +308,12 @@ hs_presto_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
     Direct d;
     load_direct<L>(d, x, frac_row(16), frac_row(8), N, nw + 16 * lane + 8 * half, nw / 2 + 8 * lane + 4 * half,
                    nw / 4 + 4 * lane + 2 * half, nw + TILE + 8 <= N, (reinterpret_cast<uintptr_t>(x) & 31u) == 0);
-    if (NF > F_SMEM) mbar_wait(smem_u32(&bar), 0);
+    if (NF > F_SMEM) mbar_wait(smem_u32(&bar[0]), 0);
+    auto wait5 = [&]() { if (SPLIT && NF > F5) mbar_wait(smem_u32(&bar[1]), 0); };
     float best[8];
     int bh[8];
-    if (half == 0) chain8<L, 0, W>(sm, st, w, lane, d, best, bh);
-    else chain8<L, 8, W>(sm, st, w, lane, d, best, bh);
+    if (half == 0) chain8<L, 0, W>(sm, st, w, lane, d, best, bh, wait5);
+    else chain8<L, 8, W>(sm, st, w, lane, d, best, bh, wait5);
     const int n_out = nw + 16 * lane + 8 * half;
     const long long o = (long long)s * sh.out_stride + n_out;
     const bool oal32 = (((reinterpret_cast<uintptr_t>(io.snr + o)) | (reinterpret_cast<uintptr_t>(io.best_h + o))) & 31u) == 0;

@@ -95,7 +95,7 @@ SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (
 
 # hs_plan_set_tuning values: 0 = the library's choice, 255 = coverage kernels, others = alternative tile shapes
 GREEDY_TUNES = [0, 3, 255]
-PRESTO_TUNES = [0, 50, 52, 255]
+PRESTO_TUNES = [0, 50, 52, 53, 255]
 
 
 @pytest.mark.parametrize("tune", GREEDY_TUNES)
