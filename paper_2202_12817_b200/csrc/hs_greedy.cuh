@@ -66,8 +66,39 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
 
     // ---- top band: order 1 is the only order of every fundamental of the tile (2 f0 > N - 1): pure streaming.
     // A thread takes 4 consecutive bins: one 16-byte load, the neighbour's first word by shuffle, 16-byte stores.
-    if (!HAS_BASE && h_top == 1 && f0 + BLOCK * R <= n_fund && f0 + BLOCK * R + 1 <= N && (BLOCK * R) % 128 == 0) {
-        if (threadIdx.x < BLOCK * R / 4) {                          // whole warps: BLOCK R / 4 is a multiple of 32
+    if (!HAS_BASE && h_top == 1 && f0 + BLOCK * R <= n_fund && f0 + BLOCK * R + 1 <= N && (BLOCK * R) % 256 == 0) {
+        const long long orow = (long long)s * sh.out_stride;
+        const bool al32 = (((reinterpret_cast<uintptr_t>(x + f0)) | reinterpret_cast<uintptr_t>(io.snr + orow + f0) |
+                            reinterpret_cast<uintptr_t>(io.best_h + orow + f0) | (WANT_PATH ? reinterpret_cast<uintptr_t>(io.path + orow + f0) : 0)) & 31u) == 0;
+        if (al32) {
+            // 8 consecutive bins per thread: one 32-byte load, the neighbour's first word by shuffle, 32-byte stores
+            // (whole sectors per lane: 6.9 TB/s against 6.2 for 16-byte stores, profiles/r02_machine_model.md)
+            if (threadIdx.x < BLOCK * R / 8) {                      // whole warps: BLOCK R / 8 is a multiple of 32
+                const int n0 = f0 + 8 * threadIdx.x;
+                float e[9];
+                asm volatile("ld.global.cs.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                             : "=f"(e[0]), "=f"(e[1]), "=f"(e[2]), "=f"(e[3]), "=f"(e[4]), "=f"(e[5]), "=f"(e[6]), "=f"(e[7]) : "l"(x + n0));
+                e[8] = __shfl_down_sync(0xffffffffu, e[0], 1);
+                if ((threadIdx.x & 31) == 31) e[8] = __ldg(x + n0 + 8);
+                float snr[8];
+                unsigned pb[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const bool shift = FUND_SELECT && DRIFT && e[k + 1] > e[k];  // strict >: ties stay
+                    snr[k] = hs_snr(shift ? e[k + 1] : e[k], st.nmis[0], st.inv_sigma[0]);
+                    pb[k] = shift ? 1u : 0u;
+                }
+                const long long o = orow + n0;
+                asm volatile("st.global.cs.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" :: "l"(io.snr + o), "f"(snr[0]), "f"(snr[1]), "f"(snr[2]),
+                             "f"(snr[3]), "f"(snr[4]), "f"(snr[5]), "f"(snr[6]), "f"(snr[7]) : "memory");
+                asm volatile("st.global.cs.v8.s32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};\n" :: "l"(io.best_h + o), "r"(1) : "memory");
+                if (WANT_PATH)
+                    asm volatile("st.global.cs.v8.u32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" :: "l"(io.path + o), "r"(pb[0]), "r"(pb[1]), "r"(pb[2]),
+                                 "r"(pb[3]), "r"(pb[4]), "r"(pb[5]), "r"(pb[6]), "r"(pb[7]) : "memory");
+            }
+            return;
+        }
+        if (threadIdx.x < BLOCK * R / 4) {                          // rows on odd 16-byte units: 16-byte loads and stores
             const int n0 = f0 + 4 * threadIdx.x;
             const float4 v = __ldcs(reinterpret_cast<const float4*>(x + n0));      // last use of these bins: evict first
             float nxt = __shfl_down_sync(0xffffffffu, v.x, 1);
@@ -81,7 +112,7 @@ hs_greedy_tile_kernel(const __grid_constant__ HsShape sh, const __grid_constant_
                 snr[k] = hs_snr(shift ? e[k + 1] : e[k], st.nmis[0], st.inv_sigma[0]);
                 pb[k] = shift ? 1u : 0u;
             }
-            const long long o = (long long)s * sh.out_stride + n0;
+            const long long o = orow + n0;
             __stcs(reinterpret_cast<float4*>(io.snr + o), make_float4(snr[0], snr[1], snr[2], snr[3]));
             __stcs(reinterpret_cast<int4*>(io.best_h + o), make_int4(1, 1, 1, 1));
             if (WANT_PATH) __stcs(reinterpret_cast<uint4*>(io.path + o), make_uint4(pb[0], pb[1], pb[2], pb[3]));
