@@ -81,7 +81,8 @@ typedef enum {
     HS_ERR_INVALID_ARG = 1,
     HS_ERR_UNSUPPORTED = 2,
     HS_ERR_ALLOC = 3,
-    HS_ERR_CUDA = 4
+    HS_ERR_CUDA = 4,
+    HS_ERR_TOO_LARGE = 5      /* hs_estimate_stats_static only: the batch needs more than the built-in scratch array */
 } hs_status;
 
 enum {
@@ -165,6 +166,37 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
                             int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
                             float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream);
 int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip);   /* -1 on invalid arguments (n_clip in 0..16) */
+
+/* hs_estimate_stats for callers that CANNOT ALLOCATE device memory -- the same statistics, the same kernels, but no
+ * d_work argument: the accumulators live in an array that is part of the library image.
+ *
+ * Use it when a cudaMalloc at this point is not an option: a real-time pipeline that partitions device memory once at
+ * start-up and must not allocate (or hit the implicit device-wide synchronisation of cudaMalloc / cudaFree) while an
+ * observation is running; a plug-in whose host application owns the allocator and passes in nothing but the input and
+ * output buffers; a process packed so tightly into a memory pool that a further allocation would fail.  The caller
+ * still passes the spectra (and optional multipliers) and the two [S][H] output arrays; everything else is as in
+ * hs_estimate_stats, results included (same kernels; fp64 sums in an unspecified order, so bit-equal on exactly
+ * representable data and equal to rounding otherwise).
+ *
+ * Limit: (n_clip + 1) * n_spectra <= HS_STATIC_STATS_MAX_ROWS (4096; e.g. 1024 spectra with three rejection rounds).
+ *   Beyond it the call returns HS_ERR_TOO_LARGE and launches nothing -- use hs_estimate_stats with your own workspace,
+ *   or split the batch over several plans.
+ * Cost: HS_STATIC_STATS_MAX_BYTES (3 MiB) of device memory on every GPU on which this library is loaded, held from
+ *   load until the process exits whether or not this entry point is ever called.
+ * First call on each device: looks up the device address of the array (one cudaGetSymbolAddress, which may make the
+ *   runtime load the library's code on that device).  Make that first call during set-up, BEFORE any CUDA stream capture
+ *   is begun; later calls on that device do no such lookup.
+ * Sharing: there is ONE array per device, shared by every plan, stream and host thread, and it keeps whatever the last
+ *   call left in it.  Each call clears the part it uses on `cuda_stream` before its first kernel, so calls that are
+ *   ordered on the device (same stream, or ordered by events) are safe back to back; two calls whose kernels can overlap
+ *   on one device (different streams, different host threads, different plans) RACE on the accumulators and return
+ *   garbage -- serialise them.
+ * The call itself never calls cudaMalloc, cudaFree or any allocating routine; asynchronous on the stream. */
+#define HS_STATIC_STATS_MAX_ROWS  4096
+#define HS_STATIC_STATS_MAX_BYTES (HS_STATIC_STATS_MAX_ROWS * 32 * 3 * 8)
+hs_status hs_estimate_stats_static(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
+                                   int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
+                                   float* d_mu, float* d_sigma, void* cuda_stream);
 
 /* The same two operations with HOST buffers (any host memory; page-locked memory copies
  * fastest).  Spectra are streamed through plan-owned device staging buffers in groups of

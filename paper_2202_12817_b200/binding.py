@@ -16,7 +16,8 @@ import torch
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libhs_b200.so")
 
-HS_OK, HS_ERR_INVALID_ARG, HS_ERR_UNSUPPORTED, HS_ERR_ALLOC, HS_ERR_CUDA = range(5)
+HS_OK, HS_ERR_INVALID_ARG, HS_ERR_UNSUPPORTED, HS_ERR_ALLOC, HS_ERR_CUDA, HS_ERR_TOO_LARGE = range(6)
+HS_STATIC_STATS_MAX_ROWS = 4096      # hs_estimate_stats_static: (n_clip + 1) * n_spectra may not exceed this
 
 HS_GREEDY_NO_FUND_SELECT = 1 << 0
 HS_GREEDY_NO_DRIFT = 1 << 1
@@ -26,7 +27,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
-           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_stats_workspace_bytes", "hs_whiten", "hs_search_host",
+           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_estimate_stats_static", "hs_stats_workspace_bytes", "hs_whiten", "hs_search_host",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -81,6 +82,8 @@ def load() -> ctypes.CDLL:
     lib.hs_run_presto_dstats.restype = ctypes.c_int
     lib.hs_estimate_stats.argtypes = [vp, i32, vp, vp, i64, i64, ctypes.c_float, i32, vp, vp, vp, i64, vp]
     lib.hs_estimate_stats.restype = ctypes.c_int
+    lib.hs_estimate_stats_static.argtypes = [vp, i32, vp, vp, i64, i64, ctypes.c_float, i32, vp, vp, vp]
+    lib.hs_estimate_stats_static.restype = ctypes.c_int
     lib.hs_search_host.argtypes = [vp, vp, vp, fp, fp, fp, fp, ctypes.c_float, vp, i64, vp, vp, i64, vp]
     lib.hs_search_host.restype = ctypes.c_int
     lib.hs_whiten.argtypes = [vp, vp, vp, vp, vp]
@@ -251,6 +254,23 @@ def hs_estimate_stats(plan, greedy: bool, d_spectra: torch.Tensor, d_inv_baselin
                                  _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), n_lo, n_hi, clip_sigma, n_clip,
                                  _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"),
                                  d_work.data_ptr(), d_work.numel() * d_work.element_size(), stream), "hs_estimate_stats")
+
+
+def hs_estimate_stats_static(plan, greedy: bool, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor],
+                             n_lo: int, n_hi: int, clip_sigma: float, n_clip: int, d_mu: torch.Tensor, d_sigma: torch.Tensor,
+                             stream: Optional[int] = None) -> None:
+    """hs_estimate_stats without a workspace argument, for callers that must not allocate device memory (a pipeline
+    with a frozen memory layout, a plug-in that is handed only its inputs and outputs): the accumulators sit in a
+    3 MiB array inside the library.  (n_clip + 1) * n_spectra <= HS_STATIC_STATS_MAX_ROWS, else HsError with status
+    HS_ERR_TOO_LARGE.  One array per device: calls that overlap on the GPU race; make the first call on a device
+    before any stream capture (include/hs.h)."""
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(d_spectra.device).cuda_stream
+    _check(lib.hs_estimate_stats_static(plan, 1 if greedy else 0, _dptr(d_spectra, torch.float32, "d_spectra"),
+                                        _dptr(d_inv_baseline, torch.float32, "d_inv_baseline"), n_lo, n_hi, clip_sigma, n_clip,
+                                        _dptr(d_mu, torch.float32, "d_mu"), _dptr(d_sigma, torch.float32, "d_sigma"), stream),
+           "hs_estimate_stats_static")
 
 
 def hs_run_greedy_host(plan, h_spectra, h_inv_baseline, mu, sigma, h_snr, h_best_h, h_path=None) -> None:

@@ -706,6 +706,67 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
     return HS_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// hs_estimate_stats_static: the statistics step for callers that cannot allocate device memory.
+//
+// Who that is: code that runs where a cudaMalloc is forbidden or ruinous -- a real-time search pipeline whose
+// device memory is carved up once at start-up and then frozen, a plug-in inside a host application that owns the
+// allocator and hands out only the input and output buffers, a worker that lives inside a memory pool with no head
+// room left (cudaMalloc may then fail, or synchronise the whole device in the middle of an observation).  Such a
+// caller can provide the spectra and the [S][H] results, but not the (n_clip + 1) x S x 32 x 3 doubles of
+// accumulators hs_estimate_stats wants as d_work.  Here that workspace lives in the library image itself.
+//
+// g_stats_scratch is a file-scope __device__ array: the CUDA runtime places one copy on EVERY device that loads
+// this library and keeps it there until the process exits (HS_STATIC_STATS_MAX_BYTES = 3 MiB per device).  In
+// host code the identifier `g_stats_scratch` is only the host-side shadow of that array -- NOT a device address
+// (a kernel handed &g_stats_scratch would fault, or scribble over host memory on a system where the GPU can reach
+// it); the device address of the current device's copy comes from cudaGetSymbolAddress, asked once per device.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_stats_scratch[HS_STATIC_STATS_MAX_BYTES];
+
+namespace {
+constexpr int HS_SCRATCH_DEVICES = 64;
+std::atomic<void*> g_stats_scratch_addr[HS_SCRATCH_DEVICES];     // device address of g_stats_scratch, per device ordinal
+
+// The plan's device must be current (cudaGetSymbolAddress answers for the current device).  The first call on a
+// device may load the library's module there, which is why it has to happen outside any stream capture.
+hs_status stats_scratch_address(int device, void** out) {
+    *out = nullptr;
+    if (device >= 0 && device < HS_SCRATCH_DEVICES) {
+        void* known = g_stats_scratch_addr[device].load(std::memory_order_acquire);
+        if (known) { *out = known; return HS_OK; }
+    }
+    void* ptr = nullptr;
+    HS_CUDA(cudaGetSymbolAddress(&ptr, g_stats_scratch));
+    if (!ptr) return cuda_fail(cudaErrorInvalidSymbol);
+    if (device >= 0 && device < HS_SCRATCH_DEVICES) g_stats_scratch_addr[device].store(ptr, std::memory_order_release);
+    *out = ptr;
+    return HS_OK;
+}
+}  // namespace
+
+hs_status hs_estimate_stats_static(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
+                                   int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
+                                   float* d_mu, float* d_sigma, void* cuda_stream) {
+    if (!plan) return HS_ERR_INVALID_ARG;
+    const int64_t need = hs_stats_workspace_bytes(plan, n_clip);
+    if (need < 0) return HS_ERR_INVALID_ARG;
+    if (need > (int64_t)HS_STATIC_STATS_MAX_BYTES) return HS_ERR_TOO_LARGE;     // (n_clip + 1) * n_spectra > HS_STATIC_STATS_MAX_ROWS
+    void* scratch = nullptr;
+    {
+        DeviceGuard guard(plan->device);                 // the symbol address is a per-device answer
+        HS_CUDA(guard.err);
+        const hs_status rc = stats_scratch_address(plan->device, &scratch);
+        if (rc != HS_OK) return rc;
+    }
+    // From here on this is hs_estimate_stats with the library-owned workspace: it validates the other arguments,
+    // clears the `need` bytes it uses with a cudaMemsetAsync ON THE STREAM (the array still holds the last call's
+    // sums), and launches the same kernels.  Nothing on this path calls cudaMalloc / cudaFree or a library routine
+    // that allocates.
+    return hs_estimate_stats(plan, greedy, d_spectra, d_inv_baseline, n_lo, n_hi, clip_sigma, n_clip, d_mu, d_sigma,
+                             scratch, need, cuda_stream);
+}
+
 hs_status hs_run_greedy_host(hs_plan_t plan, const float* h_spectra, const float* h_inv_baseline, const float* mu,
                              const float* sigma, float* h_snr, int32_t* h_best_h, uint32_t* h_path) {
     if (!h_snr || !h_best_h) return HS_ERR_INVALID_ARG;
@@ -830,6 +891,7 @@ const char* hs_status_string(hs_status s) {
         case HS_ERR_UNSUPPORTED: return "HS_ERR_UNSUPPORTED: valid but unimplemented combination";
         case HS_ERR_ALLOC: return "HS_ERR_ALLOC: allocation failed";
         case HS_ERR_CUDA: return "HS_ERR_CUDA: CUDA runtime error (see hs_last_cuda_error)";
+        case HS_ERR_TOO_LARGE: return "HS_ERR_TOO_LARGE: the request exceeds the fixed scratch capacity of a no-allocation entry point";
     }
     return "unknown hs_status";
 }

@@ -37,7 +37,7 @@ def test_no_torch_types_in_header():
 
 
 def test_status_strings(lib):
-    for code, word in ((0, "HS_OK"), (1, "INVALID_ARG"), (2, "UNSUPPORTED"), (3, "ALLOC"), (4, "CUDA")):
+    for code, word in ((0, "HS_OK"), (1, "INVALID_ARG"), (2, "UNSUPPORTED"), (3, "ALLOC"), (4, "CUDA"), (5, "TOO_LARGE")):
         assert word in lib.hs_status_string(code).decode()
 
 
