@@ -601,6 +601,58 @@ def test_r14_stats_closed_forms_and_degenerate_cases(oracle_mod):
     assert np.array_equal(mu[0], 3.0 * np.arange(1, 9)) and np.all(sg == 1.0)
 
 
+def test_r14_stats_apply_the_whitening_multiplier(oracle_mod):
+    """whitening precedes the statistics.  With power-of-two multipliers on an exact-integer spectrum
+    the product x * ib is exact, so estimate_stats(x, inv_baseline=ib) must equal estimate_stats(x * ib) bit for bit
+    (greedy, simple and PRESTO forms, with rejection rounds), must differ from estimate_stats(x), and -- for the simple
+    variant -- must equal numpy moments of numpy gathers of the product (nothing of the oracle re-used)."""
+    H, S, N = 12, 2, 9000
+    x = inputs.integer_spectra(73, S, N, 40).numpy()
+    x[:, ::613] += 2000.0
+    rng = np.random.default_rng(5)
+    ib = (2.0 ** rng.integers(-1, 3, size=(S, N))).astype(np.float32)          # 0.5, 1, 2, 4
+    prod = (x * ib).astype(np.float32)
+    assert np.array_equal(prod.astype(np.float64), x.astype(np.float64) * ib.astype(np.float64))
+    n_lo, n_hi = 7, 3000
+    for greedy, flags in ((True, 0), (True, NO_DRIFT | NO_FUND_SELECT), (False, 0), (False, ALL_HARMONICS)):
+        for n_clip in (0, 2):
+            with_ib = oracle_mod.estimate_stats(x, H, flags, greedy, n_lo, n_hi, clip=2.5, n_clip=n_clip, inv_baseline=ib)
+            of_prod = oracle_mod.estimate_stats(prod, H, flags, greedy, n_lo, n_hi, clip=2.5, n_clip=n_clip)
+            plain = oracle_mod.estimate_stats(x, H, flags, greedy, n_lo, n_hi, clip=2.5, n_clip=n_clip)
+            for a, b in zip(with_ib, of_prod):
+                assert np.array_equal(a, b), (greedy, flags, n_clip)
+            assert not np.array_equal(with_ib[0][:, 0], plain[0][:, 0]), (greedy, flags, n_clip)
+    mu, sg, cnt = oracle_mod.estimate_stats(x, H, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, inv_baseline=ib)
+    for s in range(S):
+        sums = _simple_sums_numpy(prod[s], H, n_lo, n_hi)
+        for h in range(H):
+            v = sums[:, h][~np.isnan(sums[:, h])]
+            assert cnt[s, h] == v.size
+            assert mu[s, h] == np.float32(v.mean()) and abs(float(sg[s, h]) - v.std()) <= 1e-6 * v.std()
+
+
+def limits_spectrum():
+    """Eight sums that sit exactly ON the rejection limits (reading R14: a round keeps lo <= S_h(n) <= hi).
+    Order 1 of the simple sum is x[n] itself: six bins of 10, one of 6, one of 14 -> mean 10, E[x^2] = 104,
+    variance 4, deviation 2 (all exact); with clip = 2 the limits are exactly 6 and 14, the two extreme samples."""
+    x = np.zeros((1, 64), np.float32)
+    x[0, 8:16] = [10, 6, 10, 10, 14, 10, 10, 10]
+    return x, 8, 16, 2.0
+
+
+def test_r14_rejection_limits_are_inclusive(oracle_mod):
+    """DESIGN.md R14: round p keeps lo <= S <= hi.  Samples equal to a limit stay: the second round counts all eight
+    sums and returns (10, 2); an exclusive comparison would drop the 6 and the 14 and return count 6, sigma 1
+    (zero deviation).  Limits moved slightly inwards do reject them (the comparison is really made)."""
+    x, n_lo, n_hi, clip = limits_spectrum()
+    for n_clip in (0, 1, 2):
+        mu, sg, cnt = oracle_mod.estimate_stats(x, 1, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, clip=clip, n_clip=n_clip)
+        assert cnt[0, 0] == 8 and mu[0, 0] == 10.0 and sg[0, 0] == 2.0, n_clip
+    tight = 1.999                                                        # limits 6.002 and 13.998: just inside 6 and 14
+    mu, sg, cnt = oracle_mod.estimate_stats(x, 1, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, clip=tight, n_clip=1)
+    assert cnt[0, 0] == 6 and mu[0, 0] == 10.0 and sg[0, 0] == 1.0
+
+
 # ------------------------------------------------------------------------------------------
 # R15 (NEXT-4): 2-D harmonic sums over an f-fdot plane -- oracle.greedy_2d / oracle.presto_2d
 # ------------------------------------------------------------------------------------------
