@@ -132,8 +132,11 @@ hs_status hs_run_presto(hs_plan_t plan, const float* d_spectra, const float* d_i
 /* The same two operations with PER-SPECTRUM statistics that already live on the device (the output of
  * hs_estimate_stats, or the caller's own): d_mu, d_sigma are DEVICE arrays [S][H] of fp32, entry [s][h-1] for order h
  * of spectrum s; every CTA forms 1/sigma and -mu/sigma of its spectrum exactly as the host does for the by-value
- * statistics.  sigma must be > 0 (not checked: the values are never read on the host).  Otherwise as hs_run_greedy /
- * hs_run_presto: asynchronous, no allocation, no synchronisation. */
+ * statistics.  The values are never read on the host, so they cannot be rejected as hs_run_* rejects bad host
+ * statistics: an entry whose sigma is not a positive finite number, or whose mu is not finite, is replaced ON THE DEVICE
+ * by (mu, sigma) = (0, 1) for that spectrum and order (the pair hs_estimate_stats returns for an order without samples),
+ * identically in every kernel, so equal inputs give equal outputs whichever kernel variant or tile computes a bin.
+ * Otherwise as hs_run_greedy / hs_run_presto: asynchronous, no allocation, no synchronisation. */
 hs_status hs_run_greedy_dstats(hs_plan_t plan, const float* d_spectra, const float* d_inv_baseline,
                                const float* d_mu, const float* d_sigma,
                                float* d_snr, int32_t* d_best_h, uint32_t* d_path, void* cuda_stream);

@@ -57,13 +57,20 @@ __device__ __forceinline__ void st_cs(unsigned* p, unsigned v) { __stcs(p, v); }
 
 // Per-spectrum statistics (hs_run_*_dstats): the CTA forms the two constants of spectrum s from d_mu / d_sigma exactly
 // as the host does for the by-value statistics (IEEE reciprocal, one fp32 multiply) and keeps them in shared memory.
+// Unusable entries (sigma <= 0, NaN or infinite; mu NaN or infinite) are replaced by (mu, sigma) = (0, 1).
 // Must be called by every thread of the CTA.
 __device__ __forceinline__ void hs_load_dstats(HsStats& s_st, const HsIO& io, int s, int H) {
     if (threadIdx.x < HS_MAX_H) {
         float is = 1.f, nm = 0.f;
         if ((int)threadIdx.x < H) {
-            is = __fdiv_rn(1.0f, __ldg(io.d_sigma + (long long)s * H + threadIdx.x));
-            nm = -__fmul_rn(__ldg(io.d_mu + (long long)s * H + threadIdx.x), is);
+            float sg = __ldg(io.d_sigma + (long long)s * H + threadIdx.x);
+            float mu = __ldg(io.d_mu + (long long)s * H + threadIdx.x);
+            // the host path rejects such statistics (fill_stats); device arrays are never read on the host, so an
+            // order whose sigma is not a positive finite number or whose mu is not finite is normalised with (0, 1)
+            // -- what hs_stats_finish_kernel writes for an order without samples -- in every kernel alike
+            if (!(sg > 0.f) || !(sg < __int_as_float(0x7f800000)) || !(fabsf(mu) < __int_as_float(0x7f800000))) { sg = 1.f; mu = 0.f; }
+            is = __fdiv_rn(1.0f, sg);
+            nm = -__fmul_rn(mu, is);
         }
         s_st.inv_sigma[threadIdx.x] = is;
         s_st.nmis[threadIdx.x] = nm;

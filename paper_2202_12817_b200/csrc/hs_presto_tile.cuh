@@ -23,10 +23,12 @@
 //     are contiguous in global memory too: they are loaded straight into registers (LDG.256 / LDG.128) while
 //     the bulk copies are in flight, which also keeps 12 B/bin off the shared-memory pipe;
 //   * two warps share each 512-output warp tile (one takes outputs e < 8 of every lane's 16, the other e >= 8):
-//     twice the warps for the same shared memory (occupancy is set by shared memory: 29 KB per CTA at W = 2);
+//     twice the warps for the same shared memory (occupancy is set by shared memory: 28 000 B = 27.3 KB per CTA at
+//     W = 2 and H = 32, so an SM holds 8 CTAs);
 //   * a lane's 8 outputs are consecutive: they are stored from registers as whole 32-byte sectors
 //     (st.global.v8 -> STG.E.256): no transposition through shared memory, no barrier.
-// Staging, arithmetic and stores of different tiles overlap across the 7 CTAs an SM holds.
+// Staging, arithmetic and stores of different tiles overlap across the 8 CTAs an SM holds (one tile per CTA: the
+// kernel is not persistent, the grid has one CTA per tile and spectrum).
 #pragma once
 #include "hs_common.cuh"
 

@@ -94,7 +94,7 @@ SHAPES = [(1, 2), (1, 3), (2, 33), (3, 257), (2, 1000), (1, 4099), (5, 70001), (
 
 
 # hs_plan_set_tuning values: 0 = the library's choice, 255 = coverage kernels, others = alternative tile shapes
-GREEDY_TUNES = [0, 3, 255]
+GREEDY_TUNES = [0, 3, 4, 255]        # 4 = tiles in ascending order (hs_greedy_tile_kernel<128,4,false>)
 PRESTO_TUNES = [0, 50, 52, 53, 255]
 
 
@@ -127,8 +127,9 @@ def test_presto_exact_integer(hs, oracle_mod, tune, H):
 @pytest.mark.parametrize("tune", [t for t in PRESTO_TUNES if t != 255])
 @pytest.mark.parametrize("H", [8, 32])
 def test_presto_many_tiles_per_cta(hs, oracle_mod, tune, H):
-    """Enough tiles that every CTA of a persistent kernel goes round its ring of stages many times (ragged rows,
-    rows that start on odd 16-byte units), against the oracle bit for bit on exact-integer spectra."""
+    """Many tiles per row and many rows (one CTA per tile: several waves of CTAs, 8 resident per SM, on every SM),
+    ragged rows and rows that start on odd 16-byte units (N = 150001: in_stride = 150004 words, so odd rows are not
+    32-byte aligned), against the oracle bit for bit on exact-integer spectra."""
     mu, sg = _int_stats(H)
     S, N = 48, 150001
     x = inputs.integer_spectra(300 + H, S, N, 255).numpy()
@@ -199,12 +200,12 @@ def test_cfg1_both_variants(hs, oracle_mod, tune):
     assert r["bh_mismatch"] < 10
 
 
-def test_cfg2_subset(hs, oracle_mod):
-    """configs[1] shape (2^20 bins, H = 16), 6 of its 64 rows incl. rows with injected pulsars."""
+def test_cfg2_all_rows(hs, oracle_mod):
+    """configs[1] at its full size: all 64 spectra x 2^20 bins, H = 16, every output against the oracle."""
     from parity import check_greedy, check_presto
     w = inputs.workload("cfg2")
-    rows = sorted({p.spectrum for p in w.pulsars})[:4] + [0, 63]
-    x = torch.stack([inputs.generate_row(w, s, "cuda") for s in rows]).cpu().numpy()
+    x = torch.stack([inputs.generate_row(w, s, "cuda") for s in range(w.n_spectra)]).cpu().numpy()
+    assert x.shape == (64, 1 << 20)
     mu, sg = (t.numpy() for t in inputs.exp1_stats("greedy", w.H))
     s, b, p = run_greedy(hs, x, w.H, mu, sg)
     check_greedy(oracle_mod, x, w.H, mu, sg, 0, s, b, p, T=10.0)
@@ -744,6 +745,58 @@ def test_dstats_equals_by_value_statistics(hs, oracle_mod):
         hs.hs_destroy(plan)
 
 
+def test_dstats_unusable_entries_become_zero_one(hs, oracle_mod):
+    """include/hs.h (hs_run_*_dstats): a device-side sigma that is not positive and finite, or a non-finite mu, is
+    replaced by (0, 1) for that spectrum and order, in every kernel.  Against hs_run_* with the repaired statistics
+    passed by value, row by row, bit for bit; the row crosses the streaming top band (order 1 only) and the gather
+    bands, and the coverage kernels must agree with the tile kernels."""
+    H, S, N = 16, 3, 40000
+    x = inputs.generate(inputs.Workload("n", S, N, H, seed=21)).cuda()
+    for form in ("greedy", "presto"):
+        mu, sg = inputs.exp1_stats(form, H)
+        dmu, dsg = mu.repeat(S, 1).clone(), sg.repeat(S, 1).clone()
+        dsg[0, 0] = 0.0; dsg[0, 3] = -2.0; dsg[1, 1] = float("nan"); dsg[1, 7] = float("inf")
+        dmu[2, 0] = float("nan"); dmu[2, 15] = float("-inf")
+        bad = ~((dsg > 0) & torch.isfinite(dsg) & torch.isfinite(dmu))
+        fmu, fsg = dmu.clone(), dsg.clone()
+        fmu[bad] = 0.0; fsg[bad] = 1.0
+        for tune in (0, GENERIC):
+            got = [torch.empty((S, N), dtype=torch.float32, device="cuda"), torch.empty((S, N), dtype=torch.int32, device="cuda")]
+            plan = hs.hs_plan(N, S, H)
+            plan1 = hs.hs_plan(N, 1, H)
+            try:
+                hs.hs_plan_set_tuning(plan, tune); hs.hs_plan_set_tuning(plan1, tune)
+                run_d = hs.hs_run_greedy_dstats if form == "greedy" else hs.hs_run_presto_dstats
+                args = (None,) if form == "greedy" else ()
+                run_d(plan, x, None, dmu.cuda(), dsg.cuda(), got[0], got[1], *args)
+                torch.cuda.synchronize()
+                assert torch.all(got[1] >= 1) and not torch.any(torch.isnan(got[0]))
+                for s in range(S):
+                    ref = [torch.empty((1, N), dtype=torch.float32, device="cuda"), torch.empty((1, N), dtype=torch.int32, device="cuda")]
+                    run_v = hs.hs_run_greedy if form == "greedy" else hs.hs_run_presto
+                    run_v(plan1, x[s:s + 1].contiguous(), None, fmu[s], fsg[s], ref[0], ref[1], *args)
+                    torch.cuda.synchronize()
+                    assert torch.equal(got[0][s].view(torch.int32), ref[0][0].view(torch.int32)) and torch.equal(got[1][s], ref[1][0]), (form, tune, s)
+            finally:
+                hs.hs_destroy(plan); hs.hs_destroy(plan1)
+
+
+def test_estimate_stats_rejection_limits_inclusive(hs, oracle_mod):
+    """Reading R14: a round keeps lo <= S_h(n) <= hi.  The constructed spectrum of the CPU pin
+    (tests/test_oracle_pins.py::limits_spectrum: eight order-1 sums, mean 10, deviation 2, clip 2 -> the limits are
+    exactly the samples 6 and 14): the device compares its fp32 sum with the fp32-rounded limits, the oracle its fp64
+    sum -- here both are exact, so a wrong comparison direction or limit rounding on either side shows as a count of 6."""
+    from test_oracle_pins import limits_spectrum
+    x, n_lo, n_hi, clip = limits_spectrum()
+    for n_clip in (0, 1, 2):
+        for greedy, flags in ((True, NO_DRIFT | NO_FUND_SELECT), (False, 0)):       # order 1 of both forms is x[n]
+            mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, 1, flags, greedy, n_lo, n_hi, clip=clip, n_clip=n_clip)
+            mu, sg, cnt = _gpu_stats(hs, x, 1, flags, greedy, n_lo, n_hi, clip, n_clip)
+            assert cnt[0, 0] == cnt_r[0, 0] == 8 and mu[0, 0] == mu_r[0, 0] == 10.0 and sg[0, 0] == sg_r[0, 0] == 2.0
+    mu, sg, cnt = _gpu_stats(hs, x, 1, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, 1.999, 1)
+    assert cnt[0, 0] == 6 and mu[0, 0] == 10.0 and sg[0, 0] == 1.0
+
+
 # ------------------------------------------------------------------------------------------
 # NEXT-4 (reading R15): 2-D harmonic sums over an f-fdot plane
 # ------------------------------------------------------------------------------------------
@@ -1012,3 +1065,61 @@ def test_search_host_candidates_only(hs, oracle_mod, monkeypatch):
         assert np.array_equal(g[:, [0, 1, 3]].astype(np.int64), ref)
         assert np.array_equal(g[:, 2].copy().view(np.float32).astype(np.float64), ref_snr)
     assert ng2 == ng and bool((small[:, 0] >= 0).all())
+
+
+def test_search_host_with_multiplier(hs, oracle_mod, monkeypatch):
+    """hs_search_host with h_inv_baseline: power-of-two multipliers on exact-integer spectra (every product and every
+    SNR exact), several staging chunks: both candidate lists equal the definition applied to the oracle's outputs with
+    the same multiplier, and differ from the lists without it."""
+    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
+    H, S, N = 16, 12, 40000
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(17, S, N, 63)
+    g = torch.Generator(); g.manual_seed(3)
+    ib = torch.pow(2.0, torch.randint(-1, 2, (S, N), generator=g).to(torch.float32))      # 0.5, 1, 2
+    s_ref, b_ref, _ = oracle_mod.greedy(x.numpy(), H, mu, sg, 0, inv_baseline=ib.numpy())
+    q_ref, c_ref = oracle_mod.presto(x.numpy(), H, mu, sg, 0, inv_baseline=ib.numpy())
+    T = float(np.float32(min(np.sort(s_ref.ravel())[-3000], np.sort(q_ref.ravel())[-3000])))
+    cg = torch.full((1 << 18, 4), -1, dtype=torch.int32); cp = torch.full((1 << 18, 4), -1, dtype=torch.int32)
+    cg0 = torch.full((1 << 18, 4), -1, dtype=torch.int32); cp0 = torch.full((1 << 18, 4), -1, dtype=torch.int32)
+    plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+    try:
+        ng, np_ = hs.hs_search_host(plan, x.pin_memory(), ib.pin_memory(), mu, sg, mu, sg, T, cg, cp)
+        ng0, np0 = hs.hs_search_host(plan, x.pin_memory(), None, mu, sg, mu, sg, T, cg0, cp0)
+    finally:
+        hs.hs_destroy(plan)
+    assert (ng0, np0) != (ng, np_)
+    for got, n, (sr, br) in ((cg, ng, (s_ref, b_ref)), (cp, np_, (q_ref, c_ref))):
+        ref, ref_snr = oracle_mod.candidates(sr.astype(np.float32), br, T)
+        assert n == ref.shape[0] and 10 < n < got.shape[0]
+        a = got[:n].numpy()
+        a = a[np.lexsort((a[:, 1], a[:, 0]))]
+        assert np.array_equal(a[:, [0, 1, 3]].astype(np.int64), ref)
+        assert np.array_equal(a[:, 2].copy().view(np.float32).astype(np.float64), ref_snr)
+
+
+@pytest.mark.parametrize("flags,tune,kernel", [(ALL_HARMONICS, 0, "hs_presto_farey_kernel"), (ALL_HARMONICS, 2, "hs_presto_plus_kernel"),
+                                               (ALL_HARMONICS | ALL_ORDERS, 0, "hs_presto_plus_kernel"),
+                                               (ALL_HARMONICS | ALL_ORDERS, 1, "hs_presto_farey_kernel")])
+def test_presto_variants_cfg3_sized_row(hs, oracle_mod, flags, tune, kernel):
+    """PRESTO_all / PRESTO+ (PAPER.md:174, 368), both kernels of each, on rows of cfg3's length (2^22 bins, H = 32):
+    thousands of tiles per row instead of the few of the small exact-integer shapes.  Exact-integer spectrum, sampled
+    top bins (band edges, both ends of the row, random bins) computed one by one by the oracle: bit-for-bit."""
+    H, S, N = 32, 2, 1 << 22
+    mu, sg = _int_stats(H)
+    x = inputs.integer_spectra(404, S, N, 255)
+    snr = torch.empty((S, N), dtype=torch.float32, device="cuda")
+    bh = torch.empty((S, N), dtype=torch.int32, device="cuda")
+    plan = hs.hs_plan(N, S, H, N, N, 0, flags, 0)
+    try:
+        hs.hs_plan_set_tuning(plan, tune)
+        hs.hs_run_presto(plan, x.cuda(), None, mu, sg, snr, bh)
+        torch.cuda.synchronize()
+        assert hs.hs_last_kernel(plan) == kernel
+    finally:
+        hs.hs_destroy(plan)
+    bins = _sample_bins(N, np.random.default_rng(8), k=3000)
+    for row in range(S):
+        ref = oracle_mod.presto_bins(x.numpy(), H, mu, sg, np.full(bins.shape, row), bins, flags)
+        assert np.array_equal(bh[row].cpu().numpy()[bins], ref["best_h"])
+        assert np.array_equal(snr[row].cpu().numpy()[bins].astype(np.float64), ref["snr"])
