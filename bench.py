@@ -71,6 +71,11 @@ def parse_args():
     ap.add_argument("--whiten", default="pass", choices=["pass", "fused"],
                     help="red-noise workload (cfg4): pass = hs_whiten writes x * inv_baseline once and the sums read that array; "
                          "fused = every gather multiplies (two arrays read by the gather)")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the `extra` object of the default run (H sweep, NEXT-1 variants, streaming rate, cfg4 and cfg5 lines)")
+    ap.add_argument("--n-fund-div", type=int, default=1,
+                    help="diagnostic: outputs only for n < N / D (hs_plan's n_fund), e.g. 8 = the greedy gather band without "
+                         "the streaming top band, for ncu captures; bins/s then counts S * N / D bins")
     ap.add_argument("--tune-greedy", type=int, default=0)
     ap.add_argument("--tune-presto", type=int, default=0)
     return ap.parse_args()
@@ -145,7 +150,8 @@ def respawn_under_torchrun(args) -> int:
         sk.bind(("127.0.0.1", 0))
         port = sk.getsockname()[1]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")                # the communicator lines (ranks, NVLS) of a scaling run
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
     return subprocess.call(cmd, env=env)
@@ -163,6 +169,8 @@ def dist_setup(n_gpus: int):
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29511")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")         # communicator lines of a scaling run (only the timing all-reduce uses NCCL)
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         torch.cuda.set_device(local)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     return rank, local, world
@@ -237,6 +245,20 @@ def run_reference(args):
     return 0
 
 
+def child_line(argv, keys, timeout=600):
+    """Run this script once more for another workload (its own process: its own buffers) and keep `keys` of its JSON line."""
+    try:
+        out = subprocess.run([sys.executable, os.path.abspath(__file__), "--no-e2e", "--no-cpu", "--no-extra"] + argv,
+                             capture_output=True, text=True, timeout=timeout)
+        for ln in reversed(out.stdout.splitlines()):
+            if ln.startswith("{"):
+                rec = json.loads(ln)
+                return {k: rec.get(k) for k in keys}
+        return {"error": f"no JSON line (rc {out.returncode}): {out.stderr[-300:]}"}
+    except Exception as e:          # the headline line must not depend on an extra
+        return {"error": repr(e)}
+
+
 def run_cuda(args):
     import torch
     from paper_2202_12817_b200 import binding as hs
@@ -268,8 +290,9 @@ def run_cuda(args):
     gv, fs, pv = _variants(args)
     mu_g, sg_g = inputs.exp1_stats(gv, H, fs)
     mu_p, sg_p = inputs.exp1_stats(pv, H)
-    plan_g = hs.hs_plan(N, S, H, flags=args.greedy_flags, device=local)
-    plan_p = hs.hs_plan(N, S, H, flags=args.presto_flags, device=local)
+    n_out = N // max(1, args.n_fund_div)                 # outputs per spectrum (hs_plan's n_fund; N in every quoted run)
+    plan_g = hs.hs_plan(N, S, H, N, N, n_out, flags=args.greedy_flags, device=local)
+    plan_p = hs.hs_plan(N, S, H, N, N, n_out, flags=args.presto_flags, device=local)
     hs.hs_plan_set_tuning(plan_g, args.tune_greedy)     # 0 = the library's choice (diagnostic knob)
     hs.hs_plan_set_tuning(plan_p, args.tune_presto)
     stream = torch.cuda.current_stream(dev)
@@ -353,9 +376,9 @@ def run_cuda(args):
     if wpass:                       # the whitening pass belongs to each form's 16 B/bin (x and the multiplier read once)
         g_ms += w_ms if do_g else 0.0
         p_ms += w_ms if (do_p and not do_g) else 0.0
-    bins_step = float(S) * N * world
+    bins_step = float(S) * n_out * world
     n_forms = int(do_g) + int(do_p)
-    default_run = (args.forms == "both" and not args.greedy_flags and not args.presto_flags and ib is None
+    default_run = (args.n_fund_div == 1 and args.forms == "both" and not args.greedy_flags and not args.presto_flags and ib is None
                    and not args.tune_greedy and not args.tune_presto and w.name == "cfg3" and S == w.n_spectra)
     value = bins_step * args.steps / (total_ms * 1e-3)
 
@@ -437,7 +460,7 @@ def run_cuda(args):
     # ---- roofline of the dominant kernel (HBM-bound: 12 algorithmic bytes per bin and launch) ----
     peak, peak_src = measured_peak()
     dom, dom_ms = ("greedy", g_ms) if (g_ms >= p_ms or not do_p) and do_g else ("presto", p_ms)
-    alg_bytes = (BYTES_PER_BIN + (4.0 if ib is not None else 0.0)) * S * N
+    alg_bytes = (BYTES_PER_BIN + (4.0 if ib is not None else 0.0)) * S * n_out
 
     def roof(ms):
         a = alg_bytes / (ms * 1e-3) / 1e9
@@ -445,7 +468,7 @@ def run_cuda(args):
 
     ncu = _load_json(NCU_KERNELS_JSON)
     mm = _load_json(MACHINE_MODEL_JSON)
-    full_cfg3 = (w.name == "cfg3" and S == w.n_spectra and H == w.H and ib is None
+    full_cfg3 = (w.name == "cfg3" and S == w.n_spectra and H == w.H and ib is None and args.n_fund_div == 1
                  and not args.greedy_flags and not args.presto_flags)
 
     def evidence(form):
@@ -461,7 +484,8 @@ def run_cuda(args):
             return None
         floor_ms = rec["l2_to_sm_sector_bytes"] / (l2 * 1e9) * 1e3
         out = {"l2_to_sm_gbs": l2, "sector_bytes_per_launch": rec["l2_to_sm_sector_bytes"],
-               "ceiling_ms": floor_ms, "frac_of_ceiling": floor_ms / ms, "source": mm.get("source"), "capture": rec.get("capture")}
+               "ceiling_ms": floor_ms, "frac_of_ceiling": floor_ms / ms, "source": mm.get("source"), "capture": rec.get("capture"),
+               "reproducible_from_repository": mm.get("reproducible_from_repository", False)}
         if rec.get("access_form_ceiling_ms"):      # the measured rate of the kernel's own access form (L1 line requests included)
             out.update(access_form_ceiling_ms=rec["access_form_ceiling_ms"], frac_of_access_form_ceiling=rec["access_form_ceiling_ms"] / ms,
                        access_form_note=rec.get("access_form_note"))
@@ -486,6 +510,61 @@ def run_cuda(args):
     if do_p:
         roofline["per_kernel"]["presto"] = per_kernel("presto", p_ms)
 
+    # ---- extra (default run only, after the headline region): the other configurations of BASELINE.json / BASELINE.md,
+    # measured in THIS run so that every fraction quoted there has a counterpart in the driver's record ----
+    extra = None
+    if default_run and world == 1 and not args.no_extra:
+        def timed(fn, reps=3):
+            fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+
+        def entry(plan, ms, bytes_per_bin=BYTES_PER_BIN):
+            gbs = bytes_per_bin * S * N / (ms * 1e-3) / 1e9
+            return {"kernel": hs.hs_last_kernel(plan), "launch_ms": ms, "achieved": gbs, "frac": gbs / peak, "gbins_per_s": S * N / ms / 1e6}
+
+        extra = {"note": "same batch (cfg3 spectra), CUDA events, 1 warm-up + 3 launches each; frac = 12 B/bin over the same peak as the headline"}
+        # sustained streaming rate of a product kernel (hs_whiten: two 4 GiB arrays read, one written, 12 B per element, 16-byte
+        # accesses): a live second denominator beside the copy-burst peak of MEASURED_PEAKS.json, which these kernels can exceed
+        wh_ms = timed(lambda: hs.hs_whiten(plan_g, x, snr_g, snr_p, stream.cuda_stream))
+        stream_gbs = 12.0 * S * N / (wh_ms * 1e-3) / 1e9
+        extra["stream"] = {"kernel": "hs_whiten_kernel", "launch_ms": wh_ms, "gbs": stream_gbs, "bytes_per_element": 12,
+                           "note": "measured in this run (16-byte loads and stores)"}
+        sweep = {}
+        for Hs in (4, 8, 16):                       # paper Table 2's H values on the cfg3 shape
+            pg, pp = hs.hs_plan(N, S, Hs, device=local), hs.hs_plan(N, S, Hs, device=local)
+            mg, sgg = inputs.exp1_stats("greedy", Hs, True)
+            mp, sgp = inputs.exp1_stats("presto", Hs)
+            t_g = timed(lambda: hs.hs_run_greedy(pg, x, None, mg, sgg, snr_g, bh_g, None, stream.cuda_stream))
+            t_p = timed(lambda: hs.hs_run_presto(pp, x, None, mp, sgp, snr_p, bh_p, stream.cuda_stream))
+            sweep[f"H{Hs}"] = {"greedy": entry(pg, t_g), "presto": entry(pp, t_p)}
+            hs.hs_destroy(pg); hs.hs_destroy(pp)
+        extra["h_sweep"] = sweep
+        for name, gflags, pflags in (("simple", 2, None), ("presto_all", None, 4), ("presto_plus", None, 12)):   # NEXT-1 variants, H = 32
+            pl = hs.hs_plan(N, S, H, flags=(gflags if gflags is not None else pflags), device=local)
+            if gflags is not None:
+                m_, s_ = inputs.exp1_stats("simple", H, True)
+                t = timed(lambda: hs.hs_run_greedy(pl, x, None, m_, s_, snr_g, bh_g, None, stream.cuda_stream))
+            else:
+                m_, s_ = inputs.exp1_stats(name, H)
+                t = timed(lambda: hs.hs_run_presto(pl, x, None, m_, s_, snr_p, bh_p, stream.cuda_stream), reps=2)
+            extra[name] = entry(pl, t)
+            hs.hs_destroy(pl)
+        # The copy-burst peak under-measures what HBM sustains on this pool: the H = 4 / 8 PRESTO launches above move
+        # their 12 B/bin faster than it (frac > 1).  A fraction above 1 says the denominator is low, not that a kernel
+        # beat the memory; so every fraction is also given against the highest rate any launch of THIS run sustained.
+        best = max([stream_gbs] + [v[f]["achieved"] for v in sweep.values() for f in v])
+        extra["stream"]["best_observed_gbs"] = best
+        extra["stream"]["best_observed_note"] = "max over hs_whiten and the H sweep of algorithmic bytes / time in this run"
+        for form in roofline["per_kernel"].values():
+            form["frac_vs_best_observed"] = form["achieved"] / best
+        roofline["frac_vs_best_observed"] = roofline["achieved"] / best
+
     cpu = None
     if rank == 0 and not args.no_cpu:
         rows = min(args.cpu_spectra, S)
@@ -495,6 +574,13 @@ def run_cuda(args):
                          f"PRESTO {r['presto_s']:.2f} s, fp64"}
     hs.hs_destroy(plan_g)
     hs.hs_destroy(plan_p)
+    if extra is not None:
+        del x, snr_g, bh_g, snr_p, bh_p
+        torch.cuda.empty_cache()
+        extra["cfg4"] = child_line(["--workload", "cfg4", "--forms", "greedy", "--steps", "3", "--warmup", "1"],
+                                   ("config", "ms_per_step", "value", "whiten", "stats", "roofline", "gpu_launches"))
+        extra["cfg5"] = child_line(["--workload", "cfg5", "--steps", "3", "--warmup", "1"],
+                                   ("config", "ms_per_step", "value", "roofline", "gpu_launches"))
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -503,7 +589,8 @@ def run_cuda(args):
                                        {"both": "greedy (Alg. 2) + PRESTO (Alg. 1) per step", "greedy": "greedy (Alg. 2) only",
                                         "presto": "PRESTO (Alg. 1) only"}[args.forms] +
                                        (f", stats/flags {gv}/{pv} ({args.greedy_flags}/{args.presto_flags})" if args.greedy_flags or args.presto_flags else "") +
-                                       (", per-bin inverse baseline" if ib is not None else ""),
+                                       (", per-bin inverse baseline" if ib is not None else "") +
+                                       (f", DIAGNOSTIC: outputs for n < N/{args.n_fund_div} only" if args.n_fund_div != 1 else ""),
                            "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
                 "whiten": ({"source": "hs_whiten pass inside the step; its time is counted in the form's launch_ms (16 B/bin)", "ms": w_ms} if wpass else None),
@@ -511,7 +598,7 @@ def run_cuda(args):
                                      "then hs_run_*_dstats", "ms": s_ms} if est else
                           {"source": "closed-form Exp(1) statistics passed by value", "ms": 0.0}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "candidates": cand,
-                "cpu_baseline": cpu}
+                "cpu_baseline": cpu, "extra": extra}
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
