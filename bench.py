@@ -303,7 +303,8 @@ def run_cuda(args):
     if est:
         dmu_g = torch.empty((S, H), dtype=torch.float32, device=dev); dsg_g = torch.empty_like(dmu_g)
         dmu_p = torch.empty_like(dmu_g); dsg_p = torch.empty_like(dmu_g)
-        work = torch.empty(hs.hs_stats_workspace_bytes(plan_g, n_clip) // 8, dtype=torch.float64, device=dev)
+        # the large workspace: the first gather pass stores its sums, the rejection rounds stream them (include/hs.h)
+        work = torch.empty((hs.hs_stats_workspace_bytes_cached(plan_g, n_clip, N // 64, N // 32) + 7) // 8, dtype=torch.float64, device=dev)
 
     # the whitening pass writes y = x * inv_baseline once; the sums then read y alone (same bits, reading R13)
     wpass = ib is not None and args.whiten == "pass"
@@ -594,8 +595,8 @@ def run_cuda(args):
                            "seed": w.seed, "n_pulsars": len(w.pulsars), "l2": f"inputs ({S * N * 4 / 2**30:.2f} GiB) exceed L2; no flush needed" if S * N * 4 > 256 * 2**20 else "inputs fit in L2: warm-L2 numbers",
                            "parallelism": f"spectra sharded over {world} GPU(s), no collective"},
                 "whiten": ({"source": "hs_whiten pass inside the step; its time is counted in the form's launch_ms (16 B/bin)", "ms": w_ms} if wpass else None),
-                "stats": ({"source": "hs_estimate_stats inside the step (reading R14): bins [N/64, N/32), 2 rejection rounds at 3 sigma, "
-                                     "then hs_run_*_dstats", "ms": s_ms} if est else
+                "stats": ({"source": "hs_estimate_stats inside the step (reading R14): bins [N/64, N/32), 2 rejection rounds at 3 sigma "
+                                     "(one gather pass, the rounds stream the stored sums), then hs_run_*_dstats", "ms": s_ms} if est else
                           {"source": "closed-form Exp(1) statistics passed by value", "ms": 0.0}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "candidates": cand,
                 "cpu_baseline": cpu, "extra": extra}

@@ -164,11 +164,21 @@ hs_status hs_whiten(hs_plan_t plan, const float* d_spectra, const float* d_inv_b
  *   d_mu, d_sigma  [S][H] fp32 out (device): the arguments hs_run_*_dstats take
  *   d_work       device workspace of hs_stats_workspace_bytes(plan, n_clip) bytes, 8-byte aligned (zeroed by the call)
  * S_h is accumulated in fp32 as the coverage kernels do; the moments in fp64 (the order of the fp64 additions is not
- * fixed).  Asynchronous on the stream: n_clip + 1 gather passes over [n_lo, n_hi) and one tiny launch. */
+ * fixed).  Asynchronous on the stream: n_clip + 1 gather passes over [n_lo, n_hi) and one tiny launch -- or one gather
+ * pass and n_clip streaming passes when the workspace has hs_stats_workspace_bytes_cached() bytes (below). */
 hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
                             int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
                             float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream);
 int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip);   /* -1 on invalid arguments (n_clip in 0..16) */
+
+/* A larger workspace that makes the rejection rounds cheap: hs_stats_workspace_bytes(plan, n_clip) rounded up to 256 bytes
+ * plus n_spectra * H * ((n_hi - n_lo) rounded up to 4) floats.  Given at least that many bytes (and n_clip >= 1),
+ * hs_estimate_stats writes the sums S_h(n) of its first gather pass into the workspace and rounds 1 .. n_clip stream
+ * them back instead of walking every bin's orders again: one gather pass instead of n_clip + 1.  The stored values are
+ * the fp32 sums the gather forms, the comparisons and fp64 moments are the same, so the results are those of the
+ * small-workspace path (bit-equal where the moments are exact).  cfg4 (1024 x 2^21, bins [N/64, N/32), H = 32): 4 GiB.
+ * n_hi = 0 means n_bins; -1 on invalid arguments. */
+int64_t hs_stats_workspace_bytes_cached(hs_plan_t plan, int32_t n_clip, int64_t n_lo, int64_t n_hi);
 
 /* hs_estimate_stats for callers that CANNOT ALLOCATE device memory -- the same statistics, the same kernels, but no
  * d_work argument: the accumulators live in an array that is part of the library image.

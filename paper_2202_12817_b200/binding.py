@@ -27,7 +27,7 @@ HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
            "hs_find_candidates", "hs_plan_set_tuning",
-           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_estimate_stats_static", "hs_stats_workspace_bytes", "hs_whiten", "hs_search_host",
+           "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_estimate_stats_static", "hs_stats_workspace_bytes", "hs_stats_workspace_bytes_cached", "hs_whiten", "hs_search_host",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
 
@@ -90,6 +90,8 @@ def load() -> ctypes.CDLL:
     lib.hs_whiten.restype = ctypes.c_int
     lib.hs_stats_workspace_bytes.argtypes = [vp, i32]
     lib.hs_stats_workspace_bytes.restype = i64
+    lib.hs_stats_workspace_bytes_cached.argtypes = [vp, i32, i64, i64]
+    lib.hs_stats_workspace_bytes_cached.restype = i64
     lib.hs_launch_count.argtypes = [vp]
     lib.hs_launch_count.restype = i64
     lib.hs_last_kernel.argtypes = [vp]
@@ -240,6 +242,10 @@ def hs_search_host(plan, h_spectra, h_inv_baseline, mu_greedy, sigma_greedy, mu_
 
 def hs_stats_workspace_bytes(plan, n_clip: int) -> int:
     return int(load().hs_stats_workspace_bytes(plan, n_clip))
+
+
+def hs_stats_workspace_bytes_cached(plan, n_clip: int, n_lo: int, n_hi: int) -> int:
+    return int(load().hs_stats_workspace_bytes_cached(plan, n_clip, n_lo, n_hi))
 
 
 def hs_estimate_stats(plan, greedy: bool, d_spectra: torch.Tensor, d_inv_baseline: Optional[torch.Tensor],

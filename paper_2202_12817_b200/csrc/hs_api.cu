@@ -658,6 +658,19 @@ int64_t hs_stats_workspace_bytes(hs_plan_t plan, int32_t n_clip) {
     return (int64_t)(n_clip + 1) * plan->shape.n_spectra * HS_MAX_H * 3 * (int64_t)sizeof(double);
 }
 
+namespace {
+int64_t stats_cache_pitch(int64_t count) { return (count + 3) & ~(int64_t)3; }
+int64_t stats_cache_offset(int64_t accumulators) { return (accumulators + 255) & ~(int64_t)255; }
+}  // namespace
+
+int64_t hs_stats_workspace_bytes_cached(hs_plan_t plan, int32_t n_clip, int64_t n_lo, int64_t n_hi) {
+    const int64_t need = hs_stats_workspace_bytes(plan, n_clip);
+    if (need < 0) return -1;
+    if (n_hi == 0) n_hi = plan->shape.n_bins;
+    if (n_lo < 0 || n_hi > plan->shape.n_bins || n_lo > n_hi) return -1;
+    return stats_cache_offset(need) + (int64_t)plan->shape.n_spectra * plan->shape.H * stats_cache_pitch(n_hi - n_lo) * (int64_t)sizeof(float);
+}
+
 hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spectra, const float* d_inv_baseline,
                             int64_t n_lo, int64_t n_hi, float clip_sigma, int32_t n_clip,
                             float* d_mu, float* d_sigma, void* d_work, int64_t work_bytes, void* cuda_stream) {
@@ -679,17 +692,38 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
     double* acc = static_cast<double*>(d_work);
     const long long per_round = (long long)sh.n_spectra * HS_MAX_H * 3;
     const long long count = n_hi - n_lo;
+    // cached path: a workspace of hs_stats_workspace_bytes_cached() also holds the sums of the first pass, and the
+    // rejection rounds stream them back instead of gathering again (the same fp32 values, so the same results)
+    const long long cpad = stats_cache_pitch(count);
+    const bool cached = n_clip >= 1 && count > 0 && ((reinterpret_cast<uintptr_t>(d_work) + (uintptr_t)stats_cache_offset(need)) & 15u) == 0 &&
+                        work_bytes >= stats_cache_offset(need) + (int64_t)sh.n_spectra * sh.H * cpad * (int64_t)sizeof(float);
+    float* cache = cached ? reinterpret_cast<float*>(static_cast<char*>(d_work) + stats_cache_offset(need)) : nullptr;
     if (count > 0) {
         for (int r = 0; r <= n_clip; ++r) {
             for (long long s0 = 0; s0 < sh.n_spectra; s0 += HS_MAX_GRID_Y) {
                 HsShape sub = sh;
                 sub.n_spectra = (int)std::min<long long>(HS_MAX_GRID_Y, sh.n_spectra - s0);
+                const double* prev = r ? acc + (r - 1) * per_round + s0 * HS_MAX_H * 3 : nullptr;
+                double* cur = acc + r * per_round + s0 * HS_MAX_H * 3;
+                float* csub = cached ? cache + s0 * sh.H * cpad : nullptr;
+                if (cached && r > 0) {
+                    const long long n4 = std::max(1ll, count / 4);
+                    dim3 cgrid((unsigned)std::max(1ll, std::min(64ll, (n4 + 256 * 4 - 1) / (256 * 4))), (unsigned)sh.H, (unsigned)sub.n_spectra);
+                    hs_stats_cached_kernel<<<cgrid, 256, 0, stream>>>(csub, cpad, count, sh.H, (double)clip_sigma, prev, cur);
+                    plan->launches += 1;
+                    HS_CUDA(cudaGetLastError());
+                    continue;
+                }
                 HsIO io{d_spectra + s0 * sh.in_stride, d_inv_baseline ? d_inv_baseline + s0 * sh.in_stride : nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-                HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, r ? acc + (r - 1) * per_round + s0 * HS_MAX_H * 3 : nullptr,
-                              acc + r * per_round + s0 * HS_MAX_H * 3};
-                                const long long want = std::max(1ll, (count + 256 * 2 - 1) / (256 * 2));      // two groups of 32 bins per warp
+                HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, prev, cur, csub, cpad};
+                const long long want = std::max(1ll, (count + 256 * 2 - 1) / (256 * 2));      // two groups of 32 bins per warp
                 dim3 grid((unsigned)want, (unsigned)sub.n_spectra);
-                if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                if (cached) {
+                    if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                    else if (greedy) hs_stats_pass_kernel<true, false, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                    else if (d_inv_baseline) hs_stats_pass_kernel<false, true, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                    else hs_stats_pass_kernel<false, false, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                } else if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (greedy) hs_stats_pass_kernel<true, false><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (d_inv_baseline) hs_stats_pass_kernel<false, true><<<grid, 256, 0, stream>>>(sub, io, a);
                 else hs_stats_pass_kernel<false, false><<<grid, 256, 0, stream>>>(sub, io, a);
@@ -701,7 +735,7 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
     const int total = sh.n_spectra * sh.H;
     hs_stats_finish_kernel<<<(total + 255) / 256, 256, 0, stream>>>(acc + n_clip * per_round, sh.n_spectra, sh.H, d_mu, d_sigma);
     plan->launches += 1;
-    plan->last_kernel = "hs_stats_pass_kernel";
+    plan->last_kernel = cached ? "hs_stats_pass_kernel+hs_stats_cached_kernel" : "hs_stats_pass_kernel";
     HS_CUDA(cudaGetLastError());
     return HS_OK;
 }

@@ -20,6 +20,8 @@ struct HsStatsArgs {
     double clip;                   // rejection at mean -/+ clip * std
     const double* prev;            // accumulators of the round before ([S][32][3]: count, sum, sum of squares) or null
     double* acc;                   // accumulators of this round ([S][32][3]), zeroed by the caller
+    float* cache;                  // STORE: the sums of this pass are also written here, [S][H][cpad] (NaN = no sample)
+    long long cpad;                // elements between the rows of `cache` (>= n_hi - n_lo, multiple of 4)
 };
 
 // mean and population standard deviation from (count, sum, sum of squares); no fused multiply-add, so that the
@@ -37,7 +39,10 @@ __device__ __forceinline__ void hs_moments(const double* a, double& mean, double
 // the orders of its bin and leaves S_h (NaN: order not evaluated, or rejected) in the warp's [order][lane] tile of
 // shared memory; then lane h - 1 adds up the 32 entries of order h in fp64 (count, sum, sum of squares) into its own
 // registers -- a transposition instead of 20 shuffles per order -- and adds them to global memory once, at the end.
-template <bool GREEDY, bool HAS_BASE>
+// STORE (the first pass of the cached path): the tile of sums is also written to a.cache, order by order, 128 bytes per
+// warp and order, so that the rejection rounds stream S_h(n) back (hs_stats_cached_kernel) instead of walking the
+// 32 dependent orders of every bin again.
+template <bool GREEDY, bool HAS_BASE, bool STORE = false>
 __global__ void __launch_bounds__(256)
 hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a) {
     constexpr int WARPS = 8, PITCH = 33;                    // 33: both the lane-major stores and the order-major loads are conflict-free
@@ -109,6 +114,11 @@ hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a)
             }
         }
         __syncwarp();
+        if (STORE && have) {
+            float* c = a.cache + (long long)s * sh.H * a.cpad + (g * 32 + lane);
+#pragma unroll 4
+            for (int h = 0; h < sh.H; ++h) c[(long long)h * a.cpad] = tile[h * PITCH + lane];
+        }
         const float* row = tile + lane * PITCH;             // the 32 sums of order lane + 1
 #pragma unroll 8
         for (int l = 0; l < 32; ++l) {
@@ -130,6 +140,46 @@ hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a)
         const double v = s_acc[threadIdx.x / 3][threadIdx.x % 3];
         if (v != 0.0) atomicAdd(a.acc + (long long)s * HS_MAX_H * 3 + threadIdx.x, v);
     }
+}
+
+// A rejection round of the cached path: order h of spectrum s streams its row of stored sums (fp32, NaN = no sample),
+// keeps lo <= S <= hi with the limits of the round before -- the comparison and the fp64 moments of
+// hs_stats_pass_kernel, on the same fp32 values -- and adds its totals to the round's accumulators.
+// grid: (chunks, H, spectra); the additions are fp64 in an unspecified order, as in the pass kernel.
+__global__ void __launch_bounds__(256)
+hs_stats_cached_kernel(const float* __restrict__ cache, long long cpad, long long count, int H, double clip,
+                       const double* __restrict__ prev, double* __restrict__ acc) {
+    const int h = blockIdx.y, s = blockIdx.z;
+    double mean, sd;
+    hs_moments(prev + ((long long)s * HS_MAX_H + h) * 3, mean, sd);
+    const float lo = __double2float_rn(__dsub_rn(mean, __dmul_rn(clip, sd)));
+    const float hi = __double2float_rn(__dadd_rn(mean, __dmul_rn(clip, sd)));
+    const float* __restrict__ row = cache + ((long long)s * H + h) * cpad;
+    double cnt = 0.0, s1 = 0.0, s2 = 0.0;
+    auto take = [&](float v) {
+        if (v >= lo && v <= hi) {                           // false for NaN
+            const double dv = (double)v;
+            cnt += 1.0; s1 += dv; s2 += __dmul_rn(dv, dv);
+        }
+    };
+    const long long n4 = count >> 2;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) {
+        const float4 q = __ldcs(reinterpret_cast<const float4*>(row) + i);
+        take(q.x); take(q.y); take(q.z); take(q.w);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (count & 3)) take(row[(n4 << 2) + threadIdx.x]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+        s1 += __shfl_down_sync(0xffffffffu, s1, o);
+        s2 += __shfl_down_sync(0xffffffffu, s2, o);
+    }
+    __shared__ double s_acc[3];
+    if (threadIdx.x < 3) s_acc[threadIdx.x] = 0.0;
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0 && cnt != 0.0) { atomicAdd(&s_acc[0], cnt); atomicAdd(&s_acc[1], s1); atomicAdd(&s_acc[2], s2); }
+    __syncthreads();
+    if (threadIdx.x < 3 && s_acc[threadIdx.x] != 0.0) atomicAdd(acc + ((long long)s * HS_MAX_H + h) * 3 + threadIdx.x, s_acc[threadIdx.x]);
 }
 
 // mu[s][h], sigma[s][h] from the accumulators of the last round: no samples -> (0, 1); zero deviation -> sigma 1

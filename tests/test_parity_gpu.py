@@ -637,7 +637,7 @@ def test_cfg4_full_size(hs, oracle_mod):
 # ------------------------------------------------------------------------------------------
 # NEXT-2: hs_estimate_stats (reading R14 of GetMeanStdev) and the per-spectrum statistics entry points
 # ------------------------------------------------------------------------------------------
-def _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, clip, n_clip, inv_baseline=None):
+def _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, clip, n_clip, inv_baseline=None, cached=False):
     S, N = x.shape
     istr = (N + 3) & ~3
     dx = torch.zeros((S, istr), dtype=torch.float32, device="cuda")
@@ -650,10 +650,12 @@ def _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, clip, n_clip, inv_baseline=N
     sg = torch.full((S, H), float("nan"), dtype=torch.float32, device="cuda")
     plan = hs.hs_plan(N, S, H, istr, istr, 0, flags, 0)
     try:
-        work = torch.empty(hs.hs_stats_workspace_bytes(plan, n_clip) // 8, dtype=torch.float64, device="cuda")
+        nbytes = hs.hs_stats_workspace_bytes_cached(plan, n_clip, n_lo, n_hi) if cached else hs.hs_stats_workspace_bytes(plan, n_clip)
+        work = torch.empty((nbytes + 7) // 8, dtype=torch.float64, device="cuda")
         hs.hs_estimate_stats(plan, greedy, dx, db, n_lo, n_hi, clip, n_clip, mu, sg, work)
         torch.cuda.synchronize()
-        last = work.view(n_clip + 1, S, 32, 3)[n_clip, :, :H, 0].cpu().numpy().astype(np.int64)
+        assert ("hs_stats_cached_kernel" in hs.hs_last_kernel(plan)) == (cached and n_clip >= 1 and n_hi > n_lo)
+        last = work[:(n_clip + 1) * S * 96].view(n_clip + 1, S, 32, 3)[n_clip, :, :H, 0].cpu().numpy().astype(np.int64)
     finally:
         hs.hs_destroy(plan)
     return mu.cpu().numpy(), sg.cpu().numpy(), last
@@ -670,9 +672,10 @@ def test_estimate_stats_exact_integer(hs, oracle_mod, greedy, flags):
     x[:, ::501] += 3000.0                                  # outliers for the rejection rounds
     for n_lo, n_hi, n_clip in ((0, N, 0), (77, 9000, 2), (1000, 1001, 0), (5, 5, 1)):
         mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, H, flags, greedy, n_lo, n_hi, clip=2.5, n_clip=n_clip)
-        mu, sg, cnt = _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, 2.5, n_clip)
-        assert np.array_equal(cnt, cnt_r), (n_lo, n_hi, n_clip)
-        assert np.array_equal(mu, mu_r) and np.array_equal(sg, sg_r), (n_lo, n_hi, n_clip)
+        for cached in (False, True):        # True: one gather pass, the rejection rounds stream the stored sums
+            mu, sg, cnt = _gpu_stats(hs, x, H, flags, greedy, n_lo, n_hi, 2.5, n_clip, cached=cached)
+            assert np.array_equal(cnt, cnt_r), (n_lo, n_hi, n_clip, cached)
+            assert np.array_equal(mu, mu_r) and np.array_equal(sg, sg_r), (n_lo, n_hi, n_clip, cached)
 
 
 def test_estimate_stats_red_noise_and_dstats_run(hs, oracle_mod):
@@ -690,7 +693,11 @@ def test_estimate_stats_red_noise_and_dstats_run(hs, oracle_mod):
     n_lo, n_hi = N // 64, N // 32
     for greedy in (True, False):
         mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, H, 0, greedy, n_lo, n_hi, clip=3.0, n_clip=2, inv_baseline=ib)
+        mu_c, sg_c, cnt_c = _gpu_stats(hs, x, H, 0, greedy, n_lo, n_hi, 3.0, 2, inv_baseline=ib, cached=True)
         mu, sg, cnt = _gpu_stats(hs, x, H, 0, greedy, n_lo, n_hi, 3.0, 2, inv_baseline=ib)
+        # the cached path compares the same fp32 sums with the same limits: identical counts unless a limit itself moved
+        # by the rounding of the fp64 additions' order
+        assert np.all(np.abs(cnt_c - cnt) <= 1) and np.allclose(mu_c, mu, rtol=1e-6, atol=0) and np.allclose(sg_c, sg, rtol=1e-5, atol=0)
         assert np.all(np.abs(cnt - cnt_r) <= 2)
         assert np.allclose(mu, mu_r, rtol=1e-5, atol=0) and np.allclose(sg, sg_r, rtol=1e-4, atol=0)
         if greedy:      # whitened noise: each step adds about the larger of two Exp(1)
@@ -791,10 +798,12 @@ def test_estimate_stats_rejection_limits_inclusive(hs, oracle_mod):
     for n_clip in (0, 1, 2):
         for greedy, flags in ((True, NO_DRIFT | NO_FUND_SELECT), (False, 0)):       # order 1 of both forms is x[n]
             mu_r, sg_r, cnt_r = oracle_mod.estimate_stats(x, 1, flags, greedy, n_lo, n_hi, clip=clip, n_clip=n_clip)
-            mu, sg, cnt = _gpu_stats(hs, x, 1, flags, greedy, n_lo, n_hi, clip, n_clip)
-            assert cnt[0, 0] == cnt_r[0, 0] == 8 and mu[0, 0] == mu_r[0, 0] == 10.0 and sg[0, 0] == sg_r[0, 0] == 2.0
-    mu, sg, cnt = _gpu_stats(hs, x, 1, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, 1.999, 1)
-    assert cnt[0, 0] == 6 and mu[0, 0] == 10.0 and sg[0, 0] == 1.0
+            for cached in (False, True):
+                mu, sg, cnt = _gpu_stats(hs, x, 1, flags, greedy, n_lo, n_hi, clip, n_clip, cached=cached)
+                assert cnt[0, 0] == cnt_r[0, 0] == 8 and mu[0, 0] == mu_r[0, 0] == 10.0 and sg[0, 0] == sg_r[0, 0] == 2.0
+    for cached in (False, True):
+        mu, sg, cnt = _gpu_stats(hs, x, 1, NO_DRIFT | NO_FUND_SELECT, True, n_lo, n_hi, 1.999, 1, cached=cached)
+        assert cnt[0, 0] == 6 and mu[0, 0] == 10.0 and sg[0, 0] == 1.0
 
 
 # ------------------------------------------------------------------------------------------
