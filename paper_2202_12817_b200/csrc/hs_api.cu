@@ -706,9 +706,20 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
                 const double* prev = r ? acc + (r - 1) * per_round + s0 * HS_MAX_H * 3 : nullptr;
                 double* cur = acc + r * per_round + s0 * HS_MAX_H * 3;
                 float* csub = cached ? cache + s0 * sh.H * cpad : nullptr;
-                if (cached && r > 0) {
+                if (cached && r == 0) {                      // the one gather: the sums go to the workspace
+                    HsIO io{d_spectra + s0 * sh.in_stride, d_inv_baseline ? d_inv_baseline + s0 * sh.in_stride : nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+                    HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, nullptr, nullptr, csub, cpad};
+                    dim3 sgrid((unsigned)std::max(1ll, (count + 256 * 2 - 1) / (256 * 2)), (unsigned)sub.n_spectra);   // two groups of 32 bins per warp
+                    if (greedy && d_inv_baseline) hs_stats_store_kernel<true, true><<<sgrid, 256, 0, stream>>>(sub, io, a);
+                    else if (greedy) hs_stats_store_kernel<true, false><<<sgrid, 256, 0, stream>>>(sub, io, a);
+                    else if (d_inv_baseline) hs_stats_store_kernel<false, true><<<sgrid, 256, 0, stream>>>(sub, io, a);
+                    else hs_stats_store_kernel<false, false><<<sgrid, 256, 0, stream>>>(sub, io, a);
+                    plan->launches += 1;
+                    HS_CUDA(cudaGetLastError());
+                }
+                if (cached) {
                     const long long n4 = std::max(1ll, count / 4);
-                    dim3 cgrid((unsigned)std::max(1ll, std::min(64ll, (n4 + 256 * 4 - 1) / (256 * 4))), (unsigned)sh.H, (unsigned)sub.n_spectra);
+                    dim3 cgrid((unsigned)std::max(1ll, std::min(64ll, (n4 + 256 * 16 - 1) / (256 * 16))), (unsigned)sh.H, (unsigned)sub.n_spectra);
                     hs_stats_cached_kernel<<<cgrid, 256, 0, stream>>>(csub, cpad, count, sh.H, (double)clip_sigma, prev, cur);
                     plan->launches += 1;
                     HS_CUDA(cudaGetLastError());
@@ -718,12 +729,7 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
                 HsStatsArgs a{n_lo, n_hi, (double)clip_sigma, prev, cur, csub, cpad};
                 const long long want = std::max(1ll, (count + 256 * 2 - 1) / (256 * 2));      // two groups of 32 bins per warp
                 dim3 grid((unsigned)want, (unsigned)sub.n_spectra);
-                if (cached) {
-                    if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true, true><<<grid, 256, 0, stream>>>(sub, io, a);
-                    else if (greedy) hs_stats_pass_kernel<true, false, true><<<grid, 256, 0, stream>>>(sub, io, a);
-                    else if (d_inv_baseline) hs_stats_pass_kernel<false, true, true><<<grid, 256, 0, stream>>>(sub, io, a);
-                    else hs_stats_pass_kernel<false, false, true><<<grid, 256, 0, stream>>>(sub, io, a);
-                } else if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
+                if (greedy && d_inv_baseline) hs_stats_pass_kernel<true, true><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (greedy) hs_stats_pass_kernel<true, false><<<grid, 256, 0, stream>>>(sub, io, a);
                 else if (d_inv_baseline) hs_stats_pass_kernel<false, true><<<grid, 256, 0, stream>>>(sub, io, a);
                 else hs_stats_pass_kernel<false, false><<<grid, 256, 0, stream>>>(sub, io, a);
@@ -735,7 +741,7 @@ hs_status hs_estimate_stats(hs_plan_t plan, int32_t greedy, const float* d_spect
     const int total = sh.n_spectra * sh.H;
     hs_stats_finish_kernel<<<(total + 255) / 256, 256, 0, stream>>>(acc + n_clip * per_round, sh.n_spectra, sh.H, d_mu, d_sigma);
     plan->launches += 1;
-    plan->last_kernel = cached ? "hs_stats_pass_kernel+hs_stats_cached_kernel" : "hs_stats_pass_kernel";
+    plan->last_kernel = cached ? "hs_stats_store_kernel+hs_stats_cached_kernel" : "hs_stats_pass_kernel";
     HS_CUDA(cudaGetLastError());
     return HS_OK;
 }

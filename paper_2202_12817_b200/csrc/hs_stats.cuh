@@ -20,7 +20,7 @@ struct HsStatsArgs {
     double clip;                   // rejection at mean -/+ clip * std
     const double* prev;            // accumulators of the round before ([S][32][3]: count, sum, sum of squares) or null
     double* acc;                   // accumulators of this round ([S][32][3]), zeroed by the caller
-    float* cache;                  // STORE: the sums of this pass are also written here, [S][H][cpad] (NaN = no sample)
+    float* cache;                  // hs_stats_store_kernel: the sums are written here, [S][H][cpad] (NaN = no sample)
     long long cpad;                // elements between the rows of `cache` (>= n_hi - n_lo, multiple of 4)
 };
 
@@ -39,10 +39,7 @@ __device__ __forceinline__ void hs_moments(const double* a, double& mean, double
 // the orders of its bin and leaves S_h (NaN: order not evaluated, or rejected) in the warp's [order][lane] tile of
 // shared memory; then lane h - 1 adds up the 32 entries of order h in fp64 (count, sum, sum of squares) into its own
 // registers -- a transposition instead of 20 shuffles per order -- and adds them to global memory once, at the end.
-// STORE (the first pass of the cached path): the tile of sums is also written to a.cache, order by order, 128 bytes per
-// warp and order, so that the rejection rounds stream S_h(n) back (hs_stats_cached_kernel) instead of walking the
-// 32 dependent orders of every bin again.
-template <bool GREEDY, bool HAS_BASE, bool STORE = false>
+template <bool GREEDY, bool HAS_BASE>
 __global__ void __launch_bounds__(256)
 hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a) {
     constexpr int WARPS = 8, PITCH = 33;                    // 33: both the lane-major stores and the order-major loads are conflict-free
@@ -114,11 +111,6 @@ hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a)
             }
         }
         __syncwarp();
-        if (STORE && have) {
-            float* c = a.cache + (long long)s * sh.H * a.cpad + (g * 32 + lane);
-#pragma unroll 4
-            for (int h = 0; h < sh.H; ++h) c[(long long)h * a.cpad] = tile[h * PITCH + lane];
-        }
         const float* row = tile + lane * PITCH;             // the 32 sums of order lane + 1
 #pragma unroll 8
         for (int l = 0; l < 32; ++l) {
@@ -142,7 +134,90 @@ hs_stats_pass_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a)
     }
 }
 
-// A rejection round of the cached path: order h of spectrum s streams its row of stored sums (fp32, NaN = no sample),
+// The gather of the cached path: the sums S_h(n), n in [n_lo, n_hi), h = 1..H, are written to a.cache as fp32 -- order by
+// order, 128 bytes per warp and order -- and nothing else happens here: no shared-memory tile and no moments, so the
+// kernel runs at full occupancy with two independent chains per lane (the greedy form).  Every round, the first
+// included, then streams the rows back (hs_stats_cached_kernel).  The chains are those of hs_stats_pass_kernel, term
+// for term, so the stored values are the values that kernel compares.
+template <bool GREEDY, bool HAS_BASE>
+__global__ void __launch_bounds__(256)
+hs_stats_store_kernel(const __grid_constant__ HsShape sh, HsIO io, HsStatsArgs a) {
+    constexpr int WARPS = 8, R = 2;
+    const int s = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float* __restrict__ x = io.x + (long long)s * sh.in_stride;
+    const float* __restrict__ ib = HAS_BASE ? io.inv_base + (long long)s * sh.in_stride : nullptr;
+    float* __restrict__ crow = a.cache + (long long)s * sh.H * a.cpad;
+    const float NOT = __int_as_float(0x7fc00000);           // NaN marks "no sample"
+    const long long groups = (a.n_hi - a.n_lo + 31) / 32;
+    for (long long g0 = ((long long)blockIdx.x * WARPS + warp) * R; g0 < groups; g0 += (long long)gridDim.x * WARPS * R) {
+        if (GREEDY) {
+            const long long last = sh.n_bins - 1;
+            const bool no_fs = sh.flags & HSF_NO_FUND_SELECT, no_drift = sh.flags & HSF_NO_DRIFT;
+            long long n[R], d[R];
+            float sum[R];
+            bool have[R], alive[R];
+#pragma unroll
+            for (int j = 0; j < R; ++j) {
+                n[j] = a.n_lo + (g0 + j) * 32 + lane;
+                have[j] = n[j] < a.n_hi;
+                alive[j] = have[j]; d[j] = 0; sum[j] = 0.f;
+            }
+            for (int h = 1; h <= sh.H; ++h) {
+                float av[R], bv[R];
+#pragma unroll
+                for (int j = 0; j < R; ++j) {
+                    const long long m = (long long)h * n[j] + d[j];
+                    alive[j] = alive[j] && m <= last;
+                    av[j] = 0.f; bv[j] = HS_NEG_INF;
+                    if (alive[j]) {
+                        av[j] = hs_load<HAS_BASE>(x, ib, m);
+                        if (m + 1 <= last && !no_drift && !(h == 1 && no_fs)) bv[j] = hs_load<HAS_BASE>(x, ib, m + 1);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < R; ++j) {
+                    if (alive[j]) {
+                        const bool shift = bv[j] > av[j];
+                        d[j] += shift;
+                        sum[j] = __fadd_rn(sum[j], shift ? bv[j] : av[j]);
+                    }
+                    if (have[j]) crow[(long long)(h - 1) * a.cpad + (n[j] - a.n_lo)] = alive[j] ? sum[j] : NOT;
+                }
+            }
+        } else {                                            // Alg. 1 family as hs_presto_generic_kernel walks it
+            const bool all_h = sh.flags & HSF_ALL_HARMONICS, all_o = sh.flags & HSF_ALL_ORDERS;
+            for (int j = 0; j < R; ++j) {
+                const long long n = a.n_lo + (g0 + j) * 32 + lane;
+                if (n >= a.n_hi) continue;
+                for (int Hp = 1; Hp <= sh.H; ++Hp) {
+                    const bool in_set = all_o || (Hp & (Hp - 1)) == 0;
+                    float sum = 0.f;
+                    if (in_set) {
+                        const unsigned den = 2u * Hp;
+                        const unsigned qn = (unsigned)n / (unsigned)Hp, rn = 2u * ((unsigned)n - qn * Hp);
+                        unsigned q = qn, r = rn + Hp;
+                        if (r >= den) { r -= den; ++q; }
+                        sum = hs_load<HAS_BASE>(x, ib, q);
+                        const int step = all_h ? 1 : 2;
+                        q += qn; r += rn;
+                        if (r >= den) { r -= den; ++q; }
+                        for (int h = 2; h <= Hp; h += step) {
+                            sum = __fadd_rn(sum, hs_load<HAS_BASE>(x, ib, q));
+                            for (int k = 0; k < step; ++k) {
+                                q += qn; r += rn;
+                                if (r >= den) { r -= den; ++q; }
+                            }
+                        }
+                    }
+                    crow[(long long)(Hp - 1) * a.cpad + (n - a.n_lo)] = in_set ? sum : NOT;
+                }
+            }
+        }
+    }
+}
+
+// A round of the cached path (the first one has no limits: prev == nullptr): order h of spectrum s streams its row of stored sums (fp32, NaN = no sample),
 // keeps lo <= S <= hi with the limits of the round before -- the comparison and the fp64 moments of
 // hs_stats_pass_kernel, on the same fp32 values -- and adds its totals to the round's accumulators.
 // grid: (chunks, H, spectra); the additions are fp64 in an unspecified order, as in the pass kernel.
@@ -150,10 +225,13 @@ __global__ void __launch_bounds__(256)
 hs_stats_cached_kernel(const float* __restrict__ cache, long long cpad, long long count, int H, double clip,
                        const double* __restrict__ prev, double* __restrict__ acc) {
     const int h = blockIdx.y, s = blockIdx.z;
-    double mean, sd;
-    hs_moments(prev + ((long long)s * HS_MAX_H + h) * 3, mean, sd);
-    const float lo = __double2float_rn(__dsub_rn(mean, __dmul_rn(clip, sd)));
-    const float hi = __double2float_rn(__dadd_rn(mean, __dmul_rn(clip, sd)));
+    float lo = HS_NEG_INF, hi = -HS_NEG_INF;
+    if (prev) {
+        double mean, sd;
+        hs_moments(prev + ((long long)s * HS_MAX_H + h) * 3, mean, sd);
+        lo = __double2float_rn(__dsub_rn(mean, __dmul_rn(clip, sd)));
+        hi = __double2float_rn(__dadd_rn(mean, __dmul_rn(clip, sd)));
+    }
     const float* __restrict__ row = cache + ((long long)s * H + h) * cpad;
     double cnt = 0.0, s1 = 0.0, s2 = 0.0;
     auto take = [&](float v) {
