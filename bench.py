@@ -455,7 +455,10 @@ def run_cuda(args):
         c1.record(stream)
         torch.cuda.synchronize()
         c_ms = c0.elapsed_time(c1) / 5
+        from paper_2202_12817_b200.sharding import sum_over_ranks
         cand = {"threshold": T, "count": int(ccnt.item()), "ms": c_ms, "read_gbs": S * N * 4 / (c_ms * 1e-3) / 1e9}
+        # N > 1: the candidate lists are the only result that crosses ranks; here their total size
+        cand["count_all_ranks"] = int(sum_over_ranks(cand["count"], dev))
         del cbuf
 
     # ---- roofline of the dominant kernel (HBM-bound: 12 algorithmic bytes per bin and launch) ----

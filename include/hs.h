@@ -54,7 +54,8 @@
  *   during the call and passed to the kernels by value (no hidden copy, no sync).
  *   Layout: row-major, spectrum s starts at element s*in_stride (inputs) / s*out_stride
  *   (outputs).  Device base pointers must be 16-byte aligned and strides multiples of 4
- *   elements.  Inputs and outputs must not alias.  hs_run_* are asynchronous on the given
+ *   elements.  No output array may overlap an input array or another output array anywhere in its
+ *   [S][stride] extent (checked on the address ranges: HS_ERR_INVALID_ARG).  hs_run_* are asynchronous on the given
  *   CUDA stream (a cudaStream_t passed as void*; NULL = the legacy default stream) and
  *   neither allocate nor block.  hs_run_*_host are synchronous: they return when the host
  *   output arrays are complete.  A plan may be reused for any number of runs but not
@@ -286,6 +287,10 @@ hs_status hs_search_host(hs_plan_t plan, const float* h_spectra, const float* h_
  * selects a kernel variant for the plan's later runs.  0 = the library's choice; 255 = the plain
  * one-thread-per-bin coverage kernels.  Every variant computes the results defined above. */
 hs_status hs_plan_set_tuning(hs_plan_t plan, uint32_t variant);
+
+/* UNSTABLE: input bytes per device staging slot of the *_host entry points (default 256 MiB; a slot holds at least one
+ * spectrum).  Must be called before the plan's first *_host call, which allocates the slots (HS_ERR_INVALID_ARG after). */
+hs_status hs_plan_set_host_slot_bytes(hs_plan_t plan, int64_t bytes);
 
 /* Number of kernels this plan has launched so far (for bench.py's gpu_launches). */
 int64_t hs_launch_count(hs_plan_t plan);

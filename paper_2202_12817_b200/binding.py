@@ -26,7 +26,7 @@ HS_PRESTO_ALL_ORDERS = 1 << 3
 HS_TUNE_GENERIC = 255        # hs_plan_set_tuning: the coverage kernels
 
 EXPORTS = ["hs_plan", "hs_run_greedy", "hs_run_presto", "hs_run_greedy_host", "hs_run_presto_host", "hs_run_both_host",
-           "hs_find_candidates", "hs_plan_set_tuning",
+           "hs_find_candidates", "hs_plan_set_tuning", "hs_plan_set_host_slot_bytes",
            "hs_plan_2d", "hs_run_greedy_2d", "hs_run_presto_2d", "hs_run_greedy_dstats", "hs_run_presto_dstats", "hs_estimate_stats", "hs_estimate_stats_static", "hs_stats_workspace_bytes", "hs_stats_workspace_bytes_cached", "hs_whiten", "hs_search_host",
            "hs_launch_count", "hs_last_kernel", "hs_destroy", "hs_status_string", "hs_last_cuda_error"]
 
@@ -68,6 +68,8 @@ def load() -> ctypes.CDLL:
     lib.hs_run_both_host.restype = ctypes.c_int
     lib.hs_plan_set_tuning.argtypes = [vp, u32]
     lib.hs_plan_set_tuning.restype = ctypes.c_int
+    lib.hs_plan_set_host_slot_bytes.argtypes = [vp, i64]
+    lib.hs_plan_set_host_slot_bytes.restype = ctypes.c_int
     lib.hs_find_candidates.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp, vp]
     lib.hs_find_candidates.restype = ctypes.c_int
     lib.hs_plan_2d.argtypes = [ctypes.POINTER(vp), i64, i32, i32, i64, i64, u32, i32]
@@ -325,6 +327,10 @@ def hs_find_candidates(plan, d_snr: torch.Tensor, d_best_h: torch.Tensor, thresh
 
 def hs_plan_set_tuning(plan, variant: int) -> None:
     _check(load().hs_plan_set_tuning(plan, int(variant)), "hs_plan_set_tuning")
+
+
+def hs_plan_set_host_slot_bytes(plan, nbytes: int) -> None:
+    _check(load().hs_plan_set_host_slot_bytes(plan, int(nbytes)), "hs_plan_set_host_slot_bytes")
 
 
 def hs_launch_count(plan) -> int:

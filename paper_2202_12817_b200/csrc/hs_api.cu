@@ -5,7 +5,6 @@
 #include <cuda_runtime.h>
 #include <algorithm>
 #include <atomic>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -52,6 +51,7 @@ struct hs_plan_s {
     int sm_count;
     int64_t launches;
     const char* last_kernel;   // name of the kernel variant launched last (hs_last_kernel)
+    long long host_slot_bytes; // input bytes per staging slot of the *_host entry points (hs_plan_set_host_slot_bytes)
     HostStage stage;
 };
 
@@ -294,8 +294,17 @@ hs_status check_device_args(const hs_plan_s* p, const float* x, const float* ib,
     if (!p || !x || !snr || !bh) return HS_ERR_INVALID_ARG;
     if (!aligned16(x) || !aligned16(snr) || !aligned16(bh) || (ib && !aligned16(ib)) || (path && !aligned16(path)))
         return HS_ERR_INVALID_ARG;
-    if ((const void*)x == (const void*)snr || (const void*)x == (const void*)bh || (const void*)snr == (const void*)bh)
-        return HS_ERR_INVALID_ARG;
+    // no two of the arrays may share a byte: [S][in_stride] inputs, [S][out_stride] outputs (4-byte elements)
+    const HsShape& sh = p->shape;
+    const uintptr_t in_bytes = (uintptr_t)sh.n_spectra * (uintptr_t)sh.in_stride * 4u, out_bytes = (uintptr_t)sh.n_spectra * (uintptr_t)sh.out_stride * 4u;
+    const void* ptr[5] = {x, ib, snr, bh, path};
+    const uintptr_t len[5] = {in_bytes, in_bytes, out_bytes, out_bytes, out_bytes};
+    for (int i = 0; i < 5; ++i)
+        for (int j = std::max(i + 1, 2); j < 5; ++j) {          // inputs may alias each other (they are only read), nothing may alias an output
+            if (!ptr[i] || !ptr[j]) continue;
+            const uintptr_t a = reinterpret_cast<uintptr_t>(ptr[i]), b = reinterpret_cast<uintptr_t>(ptr[j]);
+            if (a < b + len[j] && b < a + len[i]) return HS_ERR_INVALID_ARG;
+        }
     return HS_OK;
 }
 
@@ -325,9 +334,8 @@ hs_status ensure_stage(hs_plan_s* p, bool need_base, bool need_path, bool need_s
     HostStage& g = p->stage;
     const HsShape& sh = p->shape;
     if (!g.ready) {
-        // slot size: about 256 MiB of input per slot (HS_HOST_SLOT_MIB overrides: unstable, for tests), at least one spectrum
-        long long slot_bytes = 256ll << 20;
-        if (const char* e = std::getenv("HS_HOST_SLOT_MIB")) { const long long v = std::atoll(e); if (v > 0) slot_bytes = v << 20; }
+        // slot size: about 256 MiB of input per slot unless hs_plan_set_host_slot_bytes said otherwise; at least one spectrum
+        const long long slot_bytes = p->host_slot_bytes;
         const long long row_bytes = sh.in_stride * 4;
         long long rows = std::max(1ll, slot_bytes / std::max(1ll, row_bytes));
         rows = std::min<long long>(rows, sh.n_spectra);
@@ -496,6 +504,7 @@ hs_status hs_plan(hs_plan_t* plan, int64_t n_bins, int32_t n_spectra, int32_t H,
     p->sm_count = sms;
     p->launches = 0;
     p->last_kernel = "";
+    p->host_slot_bytes = 256ll << 20;
     *plan = p;
     return HS_OK;
 }
@@ -569,6 +578,12 @@ hs_status hs_run_presto_2d(hs_plan_t plan, const float* d_plane, const float* mu
     plan->last_kernel = "hs_presto2d_generic_kernel";
     plan->launches += 1;
     HS_CUDA(cudaGetLastError());
+    return HS_OK;
+}
+
+hs_status hs_plan_set_host_slot_bytes(hs_plan_t plan, int64_t bytes) {
+    if (!plan || bytes < 1 || plan->stage.ready) return HS_ERR_INVALID_ARG;     // the slots exist once a *_host call has run
+    plan->host_slot_bytes = bytes;
     return HS_OK;
 }
 

@@ -417,6 +417,19 @@ def test_error_behaviour(hs):
             hs.hs_run_presto(plan, x.view(-1)[1:-3].view(-1), None, mu, sg, snr, bh)     # misaligned pointer
         with pytest.raises(hs.HsError):
             hs.hs_run_greedy(plan, x, None, mu, sg, snr, snr.view(torch.int32))           # aliasing outputs
+        # overlapping but unequal ranges: the output starts inside the input array / inside the other output
+        big = torch.empty(3 * S * N, device="cuda")
+        for bad_x, bad_snr, bad_bh in ((big[:S * N].view(S, N), big[N:N + S * N].view(S, N), bh),
+                                       (x, big[:S * N].view(S, N), big[4:4 + S * N].view(S, N).view(torch.int32))):
+            with pytest.raises(hs.HsError) as e:
+                hs.hs_run_greedy(plan, bad_x, None, mu, sg, bad_snr, bad_bh)
+            assert e.value.status == hs.HS_ERR_INVALID_ARG
+            with pytest.raises(hs.HsError):
+                hs.hs_run_presto(plan, bad_x, None, mu, sg, bad_snr, bad_bh)
+        hs.hs_run_greedy(plan, big[:S * N].view(S, N), None, mu, sg, big[S * N:2 * S * N].view(S, N), bh)   # adjacent, not overlapping: fine
+        hs.hs_plan_set_host_slot_bytes(plan, 1 << 20)
+        with pytest.raises(hs.HsError):
+            hs.hs_plan_set_host_slot_bytes(plan, 0)
         hs.hs_run_greedy(plan, x, None, mu, sg, snr, bh)                                   # the plan is still usable
         torch.cuda.synchronize()
         assert torch.all(bh >= 1)
@@ -1017,10 +1030,9 @@ def test_more_than_65535_spectra(hs, oracle_mod):
 
 def test_host_path_many_slots_and_both_forms(hs, oracle_mod, monkeypatch):
     """The host entry points stream the batch through two staging slots on two streams: with a 1 MiB slot
-    (HS_HOST_SLOT_MIB, unstable test knob) 20 spectra of 40 000 bins take four chunks, so slots are re-used while the
+    (hs_plan_set_host_slot_bytes, unstable knob) 20 spectra of 40 000 bins take four chunks, so slots are re-used while the
     other stream is busy.  hs_run_both_host (one upload, both forms), with multiplier and path, against the oracle bit
     for bit on exact integers."""
-    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
     H, S, N = 16, 20, 40000
     mu, sg = _int_stats(H)
     x = inputs.integer_spectra(15, S, N, 63)
@@ -1033,6 +1045,7 @@ def test_host_path_many_slots_and_both_forms(hs, oracle_mod, monkeypatch):
     snr_p = pin(torch.empty((S, N), dtype=torch.float32)); bh_p = pin(torch.empty((S, N), dtype=torch.int32))
     for use_ib in (False, True):
         plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+        hs.hs_plan_set_host_slot_bytes(plan, 1 << 20)        # 1 MiB slots: several staging chunks
         try:
             hs.hs_run_both_host(plan, hx, hib if use_ib else None, mu, sg, snr_g, bh_g, path, mu, sg, snr_p, bh_p)
             assert hs.hs_launch_count(plan) >= 8            # four chunks x two forms
@@ -1050,7 +1063,6 @@ def test_search_host_candidates_only(hs, oracle_mod, monkeypatch):
     """hs_search_host: one upload, both forms, threshold + compaction on the device, only the lists come back.  Against the
     plain definition applied to the oracle's outputs (exact integers, so every snr is exact), several staging chunks,
     and a capacity smaller than the list."""
-    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
     H, S, N = 16, 20, 40000
     mu, sg = _int_stats(H)
     x = inputs.integer_spectra(16, S, N, 63)
@@ -1060,6 +1072,7 @@ def test_search_host_candidates_only(hs, oracle_mod, monkeypatch):
     hx = x.pin_memory()
     cg = torch.full((1 << 20, 4), -1, dtype=torch.int32); cp = torch.full((1 << 20, 4), -1, dtype=torch.int32)
     plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+    hs.hs_plan_set_host_slot_bytes(plan, 1 << 20)        # 1 MiB slots: several staging chunks
     try:
         ng, np_ = hs.hs_search_host(plan, hx, None, mu, sg, mu, sg, T, cg, cp)
         small = torch.full((5, 4), -1, dtype=torch.int32)
@@ -1080,7 +1093,6 @@ def test_search_host_with_multiplier(hs, oracle_mod, monkeypatch):
     """hs_search_host with h_inv_baseline: power-of-two multipliers on exact-integer spectra (every product and every
     SNR exact), several staging chunks: both candidate lists equal the definition applied to the oracle's outputs with
     the same multiplier, and differ from the lists without it."""
-    monkeypatch.setenv("HS_HOST_SLOT_MIB", "1")
     H, S, N = 16, 12, 40000
     mu, sg = _int_stats(H)
     x = inputs.integer_spectra(17, S, N, 63)
@@ -1092,6 +1104,7 @@ def test_search_host_with_multiplier(hs, oracle_mod, monkeypatch):
     cg = torch.full((1 << 18, 4), -1, dtype=torch.int32); cp = torch.full((1 << 18, 4), -1, dtype=torch.int32)
     cg0 = torch.full((1 << 18, 4), -1, dtype=torch.int32); cp0 = torch.full((1 << 18, 4), -1, dtype=torch.int32)
     plan = hs.hs_plan(N, S, H, N, N, 0, 0, 0)
+    hs.hs_plan_set_host_slot_bytes(plan, 1 << 20)        # 1 MiB slots: several staging chunks
     try:
         ng, np_ = hs.hs_search_host(plan, x.pin_memory(), ib.pin_memory(), mu, sg, mu, sg, T, cg, cp)
         ng0, np0 = hs.hs_search_host(plan, x.pin_memory(), None, mu, sg, mu, sg, T, cg0, cp0)
