@@ -60,6 +60,7 @@ def _load():
                                                  ctypes.c_double, i32, c_f, c_f, c_i64]
         lib.hs_oracle_greedy_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, c_u32, i64, i32, i32, i32]
         lib.hs_oracle_presto_2d.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, c_d, c_i32, i64, i32, i32, i32]
+        lib.hs_oracle_2d_bins.argtypes = [c_f, i64, i32, i64, i32, c_f, c_f, u32, i32, c_i64, c_i64, i64, c_d, c_i32, c_d]
         lib.hs_oracle_round_half_up.argtypes = [i64, i64]
         lib.hs_oracle_round_half_up.restype = i64
         lib.hs_oracle_presto_index.argtypes = [i32, i32, i64]
@@ -229,6 +230,26 @@ def greedy_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int]
     if rc != 0:
         raise ValueError("hs_oracle_greedy_2d: invalid arguments")
     return snr, bh, path
+
+
+def bins_2d(plane, H: int, mu, sigma, zi, r, flags: int = 0, greedy: bool = True):
+    """R15 for selected (row zi = z + Z, column r) pairs.  Returns dict(snr, best_h, snr_h [count, H]); snr_h is NaN for
+    the orders that were not evaluated."""
+    lib = _load()
+    a = _as_f32_2d(plane)
+    nz, N = a.shape
+    mu, sigma = _stats(mu, sigma, H)
+    zi = np.ascontiguousarray(np.asarray(zi, dtype=np.int64)); r = np.ascontiguousarray(np.asarray(r, dtype=np.int64))
+    if zi.shape != r.shape:
+        raise ValueError("zi/r")
+    c = zi.size
+    snr = np.empty(c, np.float64); bh = np.empty(c, np.int32); snr_h = np.empty((c, H), np.float64)
+    rc = lib.hs_oracle_2d_bins(_ptr(a, ctypes.c_float), N, nz, N, H, _ptr(mu, ctypes.c_float), _ptr(sigma, ctypes.c_float), flags,
+                               1 if greedy else 0, _ptr(zi, ctypes.c_int64), _ptr(r, ctypes.c_int64), c,
+                               _ptr(snr, ctypes.c_double), _ptr(bh, ctypes.c_int32), _ptr(snr_h, ctypes.c_double))
+    if rc != 0:
+        raise ValueError("hs_oracle_2d_bins: invalid arguments")
+    return dict(snr=snr, best_h=bh, snr_h=snr_h)
 
 
 def presto_2d(plane, H: int, mu, sigma, flags: int = 0, n_threads: Optional[int] = None, rows: Optional[Tuple[int, int]] = None):

@@ -337,8 +337,11 @@ struct Plane {
     double at(int64_t z, int64_t r) const { return (double)p[(z + Z) * stride + r]; }
 };
 
+// snr_h (nullable): the SNR of every order, NaN for the orders that were not evaluated -- for the near-tie rule of the
+// parity tests only; nothing of the sum depends on it
 void greedy2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64_t r, int64_t z,
-                  double* best_out, int32_t* besth_out, uint32_t* path_out) {
+                  double* best_out, int32_t* besth_out, uint32_t* path_out, double* snr_h = nullptr) {
+    if (snr_h) for (int h = 0; h < H; ++h) snr_h[h] = std::numeric_limits<double>::quiet_NaN();
     int64_t dr = 0, dz = 0;
     double sum = 0.0, best = NEG_INF;
     int32_t bh = 0;
@@ -356,6 +359,7 @@ void greedy2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64
         if (pick & 2) { dz += 1; path |= 1u << (16 + h - 1); }
         sum += c[pick];
         const double s = st.snr(sum, h);
+        if (snr_h) snr_h[h - 1] = s;
         if (s > best) { best = s; bh = h; }
     }
     *best_out = best; *besth_out = bh;
@@ -363,7 +367,8 @@ void greedy2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64
 }
 
 void presto2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64_t r, int64_t z,
-                  double* best_out, int32_t* besth_out) {
+                  double* best_out, int32_t* besth_out, double* snr_h = nullptr) {
+    if (snr_h) for (int h = 0; h < H; ++h) snr_h[h] = std::numeric_limits<double>::quiet_NaN();
     double best = NEG_INF;
     int32_t bh = 0;
     for (int Hp = 1; Hp <= H; ++Hp) {
@@ -372,11 +377,29 @@ void presto2d_bin(const Plane& pl, int H, const Stats& st, uint32_t flags, int64
         const int step = (flags & F_ALL_HARMONICS) ? 1 : 2;
         for (int k = 2; k <= Hp; k += step) sum += pl.at(round_half_up((int64_t)k * z, Hp), round_half_up((int64_t)k * r, Hp));
         const double s = st.snr(sum, Hp);
+        if (snr_h) snr_h[Hp - 1] = s;
         if (s > best) { best = s; bh = Hp; }
     }
     *best_out = best; *besth_out = bh;
 }
 }  // namespace
+
+// The two 2-D forms for selected (row zi = z + Z, column r) pairs, with the SNR of every order ([count][H], NaN where an
+// order was not evaluated): what the parity tests need to apply the near-tie rule on a plane.
+int hs_oracle_2d_bins(const float* plane, int64_t N, int32_t n_z, int64_t stride, int32_t H, const float* mu, const float* sigma,
+                      uint32_t flags, int32_t greedy, const int64_t* zi, const int64_t* r, int64_t count,
+                      double* snr, int32_t* best_h, double* snr_h) {
+    if (bad_common(plane, N, n_z, H, mu, sigma) || H > 16 || !(n_z & 1) || !zi || !r || !snr || !best_h || !snr_h || stride < N) return 1;
+    if (!greedy && (flags & F_ALL_ORDERS) && !(flags & F_ALL_HARMONICS)) return 1;
+    const Stats st{mu, sigma};
+    const Plane pl{plane, N, stride, (n_z - 1) / 2};
+    for (int64_t i = 0; i < count; ++i) {
+        if (zi[i] < 0 || zi[i] >= n_z || r[i] < 0 || r[i] >= N) return 1;
+        if (greedy) greedy2d_bin(pl, H, st, flags, r[i], zi[i] - pl.Z, &snr[i], &best_h[i], nullptr, snr_h + i * H);
+        else presto2d_bin(pl, H, st, flags, r[i], zi[i] - pl.Z, &snr[i], &best_h[i], snr_h + i * H);
+    }
+    return 0;
+}
 
 // plane: [n_z][stride] fp32, n_z odd; outputs [n_z][out_stride], only rows zi_lo <= z + Z < zi_hi are computed and
 // written (the sums still read the whole plane); H <= 16.  Returns 0, or 1 on invalid arguments.

@@ -765,3 +765,39 @@ def test_r15_drifting_delta_train_and_truncation(oracle_mod):
             n_r = H if r == 0 else min(H, (N - 1) // r)
             n_z = H if z == 0 else min(H, Z // abs(z))
             assert b[z + Z, r] == min(n_r, n_z), (z, r)
+
+
+def test_r15_bins_entry_agrees_with_the_plane_functions_and_exposes_every_order(oracle_mod):
+    """oracle.bins_2d (per-order SNRs for the near-tie rule of the GPU tests) against what is already pinned: its snr and
+    best_h equal greedy_2d / presto_2d at the same (z, r); best is the FIRST maximum of its per-order list (strict >);
+    the orders that are NaN are exactly those the definition does not evaluate (k r > N - 1 or |k z| > Z for the simple
+    sum; orders outside the set {1, 2, 4, ..} for the PRESTO-like form); and for the simple sum the per-order values are
+    the cumulative sums of P[k z][k r] written out in numpy."""
+    H, nz, N = 8, 9, 300
+    Z = (nz - 1) // 2
+    P = _int_plane(31, nz, N, 40)
+    mu = np.array([2.0 * h for h in range(1, H + 1)], np.float32)
+    sg = np.array([2.0 ** (h % 3) for h in range(1, H + 1)], np.float32)
+    zi, r = np.meshgrid(np.arange(nz), np.arange(N), indexing="ij")
+    zi, r = zi.ravel(), r.ravel()
+    for greedy, flags in ((True, 0), (True, NO_DRIFT), (False, 0), (False, ALL_HARMONICS)):
+        full = oracle_mod.greedy_2d(P, H, mu, sg, flags) if greedy else oracle_mod.presto_2d(P, H, mu, sg, flags)
+        b = oracle_mod.bins_2d(P, H, mu, sg, zi, r, flags, greedy)
+        assert np.array_equal(b["snr"], full[0].ravel()) and np.array_equal(b["best_h"], full[1].ravel())
+        sh = b["snr_h"]
+        filled = np.where(np.isnan(sh), -np.inf, sh)
+        assert np.array_equal(filled.max(axis=1), b["snr"])
+        assert np.array_equal(filled.argmax(axis=1) + 1, b["best_h"])            # numpy's argmax is the first maximum
+        if not greedy:
+            in_set = np.array([(flags & ALL_ORDERS) or (h & (h - 1)) == 0 for h in range(1, H + 1)])
+            assert np.all(np.isnan(sh[:, ~in_set])) and not np.any(np.isnan(sh[:, in_set]))
+        if greedy and flags == NO_DRIFT:
+            z = zi - Z
+            run = np.zeros(zi.size); alive = np.ones(zi.size, bool)
+            for k in range(1, H + 1):
+                alive &= (k * r <= N - 1) & (np.abs(k * z) <= Z)
+                run[alive] += P[(k * z + Z)[alive], (k * r)[alive]]
+                want = (run - float(mu[k - 1])) / float(sg[k - 1])
+                assert np.array_equal(np.isnan(sh[:, k - 1]), ~alive)
+                assert np.array_equal(sh[alive, k - 1], want[alive])
+
