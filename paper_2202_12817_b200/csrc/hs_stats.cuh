@@ -283,6 +283,26 @@ hs_whiten_kernel(const float* __restrict__ x, const float* __restrict__ ib, floa
     const float* xr = x + (long long)s * in_stride;
     const float* br = ib + (long long)s * in_stride;
     float* yr = y + (long long)s * y_stride;
+    // rows on 32-byte units: 32-byte loads and stores (whole sectors per lane), the remainder below as before
+    if ((((reinterpret_cast<uintptr_t>(xr)) | reinterpret_cast<uintptr_t>(br) | reinterpret_cast<uintptr_t>(yr)) & 31u) == 0) {
+        const int n8 = n_bins >> 3;
+        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += gridDim.x * blockDim.x) {
+            float a[8], b[8];
+            asm volatile("ld.global.cs.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                         : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]), "=f"(a[4]), "=f"(a[5]), "=f"(a[6]), "=f"(a[7]) : "l"(xr + 8ll * i));
+            asm volatile("ld.global.cs.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                         : "=f"(b[0]), "=f"(b[1]), "=f"(b[2]), "=f"(b[3]), "=f"(b[4]), "=f"(b[5]), "=f"(b[6]), "=f"(b[7]) : "l"(br + 8ll * i));
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = __fmul_rn(a[k], b[k]);
+            asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" :: "l"(yr + 8ll * i), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]),
+                         "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+        }
+        if (blockIdx.x == 0 && threadIdx.x < (n_bins & 7)) {
+            const int i = (n8 << 3) + threadIdx.x;
+            yr[i] = __fmul_rn(__ldg(xr + i), __ldg(br + i));
+        }
+        return;
+    }
     const int n4 = n_bins >> 2;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
         const float4 a = __ldcs(reinterpret_cast<const float4*>(xr) + i);
