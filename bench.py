@@ -581,6 +581,27 @@ def run_cuda(args):
     if extra is not None:
         del x, snr_g, bh_g, snr_p, bh_p
         torch.cuda.empty_cache()
+        # the paper's Table 2 shape (1024 spectra x 131 072 bins, pure noise), H = 32 / 16 / 8 / 4: context for
+        # BASELINE.md's comparison table; 512 MiB of spectra, so partly L2-warm between launches (said in the entry)
+        wp = inputs.workload("cfgP")
+        Sp, Np = wp.n_spectra, wp.n_bins
+        xp = torch.empty((Sp, Np), dtype=torch.float32, device=dev)
+        for srow in range(Sp):
+            xp[srow].copy_(inputs.generate_row(wp, srow, dev))
+        o_s = torch.empty((Sp, Np), dtype=torch.float32, device=dev); o_b = torch.empty((Sp, Np), dtype=torch.int32, device=dev)
+        cfgp = {"note": f"{Sp} x {Np} fp32 bins (paper's Table 2 shape), 1 warm-up + 3 launches, partly L2-warm; frac = 12 B/bin over the measured peak"}
+        for Hs in (32, 16, 8, 4):
+            pg, pp = hs.hs_plan(Np, Sp, Hs, device=local), hs.hs_plan(Np, Sp, Hs, device=local)
+            mg, sgg = inputs.exp1_stats("greedy", Hs, True)
+            mp, sgp = inputs.exp1_stats("presto", Hs)
+            t_g = timed(lambda: hs.hs_run_greedy(pg, xp, None, mg, sgg, o_s, o_b, None, stream.cuda_stream))
+            t_p = timed(lambda: hs.hs_run_presto(pp, xp, None, mp, sgp, o_s, o_b, stream.cuda_stream))
+            cfgp[f"H{Hs}"] = {f: {"launch_ms": t, "gbins_per_s": Sp * Np / t / 1e6, "frac": 12.0 * Sp * Np / (t * 1e-3) / 1e9 / peak}
+                              for f, t in (("greedy", t_g), ("presto", t_p))}
+            hs.hs_destroy(pg); hs.hs_destroy(pp)
+        extra["cfgP"] = cfgp
+        del xp, o_s, o_b
+        torch.cuda.empty_cache()
         extra["cfg4"] = child_line(["--workload", "cfg4", "--forms", "greedy", "--steps", "3", "--warmup", "1"],
                                    ("config", "ms_per_step", "value", "whiten", "stats", "roofline", "gpu_launches"))
         extra["cfg5"] = child_line(["--workload", "cfg5", "--steps", "3", "--warmup", "1"],
